@@ -1,0 +1,141 @@
+/* echo.h — C ABI of libecho_b200: one explicit time step of 3-D special-relativistic ideal MHD
+ * (the ECHO scheme of arXiv:2401.03008) on a uniform periodic Cartesian unit box, FP64, as
+ * hand-written CUDA kernels for sm_100a.
+ *
+ * Citations: "P:L<n>" = line n of the paper text; "O1".."O9", "S1".."S19" = the
+ * readings of the paper recorded in DESIGN.md (same labels as SURVEY.md §8(c)).
+ *
+ * Conventions (all calls)
+ *   - extern "C", opaque handle, plain pointers and sizes; no exceptions cross the ABI.
+ *   - Unless a parameter says "host", every array pointer is a DEVICE pointer to a caller-owned
+ *     FP64 buffer of N = nx*ny*nz elements, x fastest: index = i + nx*(j + ny*k).  The
+ *     library never frees caller memory and keeps no pointer beyond the call, except the
+ *     workspace and the stream given to echo_bind.
+ *   - Staggering: cell (i,j,k) is centred at ((i+1/2)/nx, (j+1/2)/ny, (k+1/2)/nz); a face array
+ *     Bd[i,j,k] is the point value of B_d at the d-face on the + side of the cell; an edge
+ *     array Ek[i,j,k] sits at the k-edge displaced +1/2 in the two other directions.  All indices
+ *     wrap periodically; there are no ghost cells.
+ *   - Calls enqueue work on the bound CUDA stream and do NOT synchronise unless stated.
+ *   - Return value: ECHO_OK (0) or a negative ECHO_E* code; echo_last_error(ctx) gives a message.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns ECHO_ECUDA.
+ */
+#ifndef ECHO_B200_H
+#define ECHO_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ECHO_OK 0
+#define ECHO_EINVAL (-1) /* bad argument or size */
+#define ECHO_ENOMEM (-2) /* workspace missing or too small */
+#define ECHO_ECUDA (-3)  /* CUDA runtime error (message in echo_last_error) */
+#define ECHO_ESTATE (-4) /* called before echo_bind / echo_set_primitives */
+#define ECHO_EC2P (-5)   /* at least one cell failed the conservative->primitive inversion */
+
+#define ECHO_NDIAG 24
+
+typedef struct echo_ctx echo_ctx;
+
+/* Host only.  Periodic unit box of nx*ny*nz cells (each >= 1; a size-1 axis is legal and makes
+ * the problem 2-D / 1-D through the periodic wrap), ideal-gas index gamma > 1 (eq.(6)),
+ * Courant number cfl > 0 (dt = cfl * min_d h_d / a_max, S9).  Returns NULL on bad arguments. */
+echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl);
+
+/* Host only.  Frees the handle (never the workspace). */
+void echo_destroy(echo_ctx *ctx);
+
+/* Host only.  Bytes of device workspace the handle needs (44 fields of N doubles + control block,
+ * DESIGN.md "Data layout in HBM"). */
+size_t echo_workspace_bytes(const echo_ctx *ctx);
+
+/* Binds a caller-owned device workspace (256-byte aligned, >= echo_workspace_bytes) and a CUDA
+ * stream (cudaStream_t passed as void*; NULL = default stream).  The workspace must outlive the
+ * handle.  Zero-fills the control block.  ECHO_ENOMEM if too small or misaligned. */
+int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
+
+/* Message of the last error on this handle (host string owned by the handle; "" if none). */
+const char *echo_last_error(const echo_ctx *ctx);
+
+/* Initial data: cell-centred rho, v, p and FACE-staggered B point values.  Computes the centred B
+ * by INT (O1) and the conserved variables by prim2cons (definitions);
+ * sets t = 0, steps = 0.  The caller is responsible for divergence-free faces (S11). */
+int echo_set_primitives(echo_ctx *ctx, const double *rho, const double *vx, const double *vy,
+                        const double *vz, const double *p, const double *bx_face,
+                        const double *by_face, const double *bz_face);
+
+/* Same, from HOST buffers (pageable or pinned): eight cudaMemcpyAsync host->device into workspace
+ * scratch, then echo_set_primitives.  Used by the end-to-end measurement. */
+int echo_set_primitives_host(echo_ctx *ctx, const double *rho, const double *vx, const double *vy,
+                             const double *vz, const double *p, const double *bx_face,
+                             const double *by_face, const double *bz_face);
+
+/* Staggered B from an edge-centred vector potential (S11): B = curl A with the same DER-corrected
+ * discrete curl as the induction equation (O8, eq.(10)), so that echo_div_b of the result
+ * vanishes to round-off; then adds the uniform field (b0x,b0y,b0z).  ax/ay/az are edge arrays,
+ * bx/by/bz face arrays (outputs), all device. */
+int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay, const double *az,
+                              double b0x, double b0y, double b0z, double *bx_face, double *by_face,
+                              double *bz_face);
+
+/* Advances nsteps full SSP-RK3 steps (O9; five points of a sub-step), or fewer if t
+ * reaches t_end: the last dt is clipped to t_end - t on the device and later steps are no-ops
+ * (pass +inf to disable).  The time step is formed on the device from the stage-1 characteristic
+ * speeds of the same step (S9).  No host synchronisation. */
+int echo_step(echo_ctx *ctx, int nsteps, double t_end);
+
+/* Runs INT + con2prim on the current state and writes the 8 cell-centred fields; the three face
+ * pointers may be NULL.  Does not synchronise.  (con2prim failures are reported by
+ * echo_diagnostics, not here, because that would need a synchronisation.) */
+int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p,
+                        double *bx_c, double *by_c, double *bz_c, double *bx_face, double *by_face,
+                        double *bz_face);
+
+/* Same into HOST buffers; synchronises the stream before returning. */
+int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz,
+                             double *p, double *bx_c, double *by_c, double *bz_c, double *bx_face,
+                             double *by_face, double *bz_face);
+
+/* Copies the 5 conserved cell fields D, Sx, Sy, Sz, U of the current state (device). */
+int echo_get_conserved(echo_ctx *ctx, double *D, double *Sx, double *Sy, double *Sz, double *U);
+
+/* Spatial operator L(U) of eq.(9)-(10) for the current state, without changing it:
+ * rhsU[5] cell arrays, rhsB[3] face arrays, E[3] edge arrays (O7); any of the three pointer
+ * tables (HOST arrays of DEVICE pointers) may be NULL.  amax_host (host, may be NULL) receives
+ * the maximum characteristic speed (a8); synchronises if amax_host != NULL. */
+int echo_rhs(echo_ctx *ctx, double *const *rhsU, double *const *rhsB, double *const *E,
+             double *amax_host);
+
+/* Stateless batched conservative->primitive inversion (O2, "iterative Newton scheme") of n
+ * independent states on the given stream (void* cudaStream_t).  iters[i] (device int array, may
+ * be NULL) = Newton updates applied, negative on failure (outputs NaN).  Does not synchronise. */
+int echo_con2prim(double gamma, long n, const double *D, const double *Sx, const double *Sy,
+                  const double *Sz, const double *U, const double *Bx, const double *By,
+                  const double *Bz, double *rho, double *vx, double *vy, double *vz, double *p,
+                  int *iters, void *cuda_stream);
+
+/* Stateless batched primitive->conservative map. */
+int echo_prim2cons(double gamma, long n, const double *rho, const double *vx, const double *vy,
+                   const double *vz, const double *p, const double *Bx, const double *By,
+                   const double *Bz, double *D, double *Sx, double *Sy, double *Sz, double *U,
+                   void *cuda_stream);
+
+/* High-order divergence sum_d (DER_d(B_d)_{+1/2} - DER_d(B_d)_{-1/2})/h_d at cell centres (S10),
+ * the one UCT preserves.  div_field (device, N doubles) may be NULL; max_abs_host (host)
+ * may be NULL.  Synchronises. */
+int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host);
+
+/* out (HOST, ECHO_NDIAG doubles) = {t, dt_last, steps, amax, sum D, sum Sx, sum Sy, sum Sz, sum U
+ * (each x cell volume), sum Bx, sum By, sum Bz over faces (x volume), max|div_HO B|, max W,
+ * min rho, min p, con2prim max iterations, con2prim mean iterations (both of the pass run by this
+ * call), con2prim failures since echo_set_primitives, 0...}.  Sums are taken in a fixed order
+ * (fixed chunks on the device, extended precision across chunks on the host) so that drift at
+ * 1e-15 is measurable.  Synchronises.  Returns ECHO_EC2P if the failure count is non-zero. */
+int echo_diagnostics(echo_ctx *ctx, double *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ECHO_B200_H */

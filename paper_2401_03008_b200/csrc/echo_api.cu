@@ -1,0 +1,421 @@
+// echo_api.cu — C-ABI layer of libecho_b200 (see include/echo.h): argument checks, workspace
+// carving, kernel launches on the bound stream.  No arithmetic of the method lives here.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/echo.h"
+#include "echo_kernels.cuh"
+
+using namespace echo;
+
+struct echo_ctx {
+    Grid g;
+    double gamma, cfl, gg, hmin;
+    char *ws = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    Ctrl *ctrl = nullptr;
+    double *part = nullptr;
+    double *field[NFIELD] = {nullptr};
+    long long npad = 0;
+    bool bound = false, has_state = false;
+    std::string err;
+};
+
+namespace {
+
+enum { F_U = 0, F_BF = 5, F_U1 = 8, F_BF1 = 13, F_P = 16, F_BC = 21, F_R = 24, F_AP = 29, F_AM = 32, F_VB = 35, F_E = 41 };
+
+int fail(echo_ctx *c, int code, const std::string &msg) {
+    if (c) c->err = msg;
+    return code;
+}
+int cuda_fail(echo_ctx *c, cudaError_t e, const char *where) {
+    return fail(c, ECHO_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);   \
+    } while (0)
+#define LAUNCH_CHECK(name)                                         \
+    do {                                                           \
+        cudaError_t e_ = cudaGetLastError();                       \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, name);    \
+    } while (0)
+
+dim3 cell_block() { return dim3(64, 4, 1); }
+dim3 cell_grid(const Grid &g) { return dim3((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]); }
+
+// which[0] -> fields of the state L is applied to (0 = U^n at F_U, 1 = stage state at F_U1)
+Stage make_stage(const echo_ctx *c, int which) {
+    Stage st;
+    const int u0 = which ? F_U1 : F_U, b0 = which ? F_BF1 : F_BF;
+    for (int v = 0; v < 5; ++v) { st.U[v] = c->field[u0 + v]; st.P[v] = c->field[F_P + v]; st.R[v] = c->field[F_R + v]; }
+    for (int d = 0; d < 3; ++d) {
+        st.Bf[d] = c->field[b0 + d];
+        st.Bc[d] = c->field[F_BC + d];
+        st.ap[d] = c->field[F_AP + d];
+        st.am[d] = c->field[F_AM + d];
+        st.vb[d][0] = c->field[F_VB + 2 * d];
+        st.vb[d][1] = c->field[F_VB + 2 * d + 1];
+        st.E[d] = c->field[F_E + d];
+    }
+    return st;
+}
+
+template <int D>
+int launch_flux(echo_ctx *ctx, const Stage &st, const int *active, int want_amax) {
+    constexpr int NT = 128;
+    constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
+    const Grid &g = ctx->g;
+    FluxTile tl;
+    const int Lmax = 64;
+    tl.T = (D == 0) ? 4 : 16;
+    tl.tilesD = (g.n[D] + Lmax - 1) / Lmax;
+    tl.L = (g.n[D] + tl.tilesD - 1) / tl.tilesD;
+    tl.tilesT = (g.n[TD] + tl.T - 1) / tl.T;
+    const size_t smem = sizeof(double) * 5 * (size_t)(tl.L + 5) * tl.T;
+    dim3 grid(tl.tilesT, tl.tilesD, g.n[OD]);
+    k_flux<D, NT><<<grid, NT, smem, ctx->stream>>>(g, st, tl, ctx->gamma, ctx->gg, ctx->ctrl, active, want_amax);
+    LAUNCH_CHECK("k_flux");
+    return ECHO_OK;
+}
+
+// points 1-4 of a sub-step on the given stage pointers
+int launch_operator(echo_ctx *ctx, const Stage &st, const int *active, int want_amax) {
+    const Grid &g = ctx->g;
+    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, active);
+    LAUNCH_CHECK("k_prim");
+    int rc;
+    if ((rc = launch_flux<0>(ctx, st, active, want_amax))) return rc;
+    if ((rc = launch_flux<1>(ctx, st, active, want_amax))) return rc;
+    if ((rc = launch_flux<2>(ctx, st, active, want_amax))) return rc;
+    if (want_amax == 2) {   // stage 1 of echo_step: dt must exist before the update (S9)
+        k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin);
+        LAUNCH_CHECK("k_set_dt");
+    }
+    k_uct<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, active);
+    LAUNCH_CHECK("k_uct");
+    return ECHO_OK;
+}
+
+int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, double c0, double c1,
+                  const int *active) {
+    Update up;
+    for (int v = 0; v < 8; ++v) {
+        up.base[v] = ctx->field[F_U + v];
+        up.cur[v] = ctx->field[(cur_which ? F_U1 : F_U) + v];
+        up.out[v] = ctx->field[(out_which ? F_U1 : F_U) + v];
+    }
+    up.c0 = c0;
+    up.c1 = c1;
+    const Grid &g = ctx->g;
+    k_update<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1], st.R[2],
+                                                             st.R[3], st.R[4], up, ctx->ctrl, active);
+    LAUNCH_CHECK("k_update");
+    return ECHO_OK;
+}
+
+int check_ready(echo_ctx *ctx, bool need_state) {
+    if (!ctx) return ECHO_EINVAL;
+    if (!ctx->bound) return fail(ctx, ECHO_ESTATE, "echo_bind has not been called");
+    if (need_state && !ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_primitives has not been called");
+    return ECHO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl) {
+    if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || !(cfl > 0.0) || !std::isfinite(gamma) || !std::isfinite(cfl))
+        return nullptr;
+    if ((long long)nx * ny * nz > (1LL << 40) || nz > 65535 || ny > 4 * 65535) return nullptr;
+    echo_ctx *c = new (std::nothrow) echo_ctx();
+    if (!c) return nullptr;
+    Grid &g = c->g;
+    g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+    g.s[0] = 1; g.s[1] = nx; g.s[2] = (long long)nx * ny;
+    g.N = (long long)nx * ny * nz;
+    for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; }
+    c->gamma = gamma;
+    c->cfl = cfl;
+    c->gg = gamma / (gamma - 1.0);
+    c->hmin = std::fmin(g.h[0], std::fmin(g.h[1], g.h[2]));
+    c->npad = (g.N + 31) / 32 * 32;
+    return c;
+}
+
+void echo_destroy(echo_ctx *ctx) { delete ctx; }
+
+size_t echo_workspace_bytes(const echo_ctx *ctx) {
+    if (!ctx) return 0;
+    return CTRL_BYTES + PART_BYTES + sizeof(double) * (size_t)ctx->npad * NFIELD;
+}
+
+const char *echo_last_error(const echo_ctx *ctx) { return ctx ? ctx->err.c_str() : "null handle"; }
+
+int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream) {
+    if (!ctx) return ECHO_EINVAL;
+    if (!dev_workspace || bytes < echo_workspace_bytes(ctx) || ((size_t)dev_workspace & 255))
+        return fail(ctx, ECHO_ENOMEM, "workspace missing, misaligned or smaller than echo_workspace_bytes");
+    ctx->ws = static_cast<char *>(dev_workspace);
+    ctx->ws_bytes = bytes;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    ctx->ctrl = reinterpret_cast<Ctrl *>(ctx->ws);
+    ctx->part = reinterpret_cast<double *>(ctx->ws + CTRL_BYTES);
+    double *f0 = reinterpret_cast<double *>(ctx->ws + CTRL_BYTES + PART_BYTES);
+    for (int f = 0; f < NFIELD; ++f) ctx->field[f] = f0 + (size_t)f * ctx->npad;
+    Ctrl h;
+    std::memset(&h, 0, sizeof(h));
+    h.one = 1;
+    CU(cudaMemcpyAsync(ctx->ctrl, &h, sizeof(h), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));   // h is a stack object
+    CU(cudaFuncSetAttribute(k_flux<0, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CU(cudaFuncSetAttribute(k_flux<1, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CU(cudaFuncSetAttribute(k_flux<2, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    ctx->bound = true;
+    ctx->has_state = false;
+    return ECHO_OK;
+}
+
+int echo_set_primitives(echo_ctx *ctx, const double *rho, const double *vx, const double *vy, const double *vz,
+                        const double *p, const double *bxf, const double *byf, const double *bzf) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    if (!rho || !vx || !vy || !vz || !p || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
+    const Grid &g = ctx->g;
+    const double *bf[3] = {bxf, byf, bzf};
+    for (int d = 0; d < 3; ++d)
+        if (bf[d] != ctx->field[F_BF + d])
+            CU(cudaMemcpyAsync(ctx->field[F_BF + d], bf[d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
+    k_init<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, rho, vx, vy, vz, p, ctx->field[F_BF], ctx->field[F_BF + 1],
+                                                           ctx->field[F_BF + 2], ctx->field[F_U], ctx->field[F_U + 1],
+                                                           ctx->field[F_U + 2], ctx->field[F_U + 3], ctx->field[F_U + 4],
+                                                           ctx->gg);
+    LAUNCH_CHECK("k_init");
+    Ctrl h;
+    std::memset(&h, 0, sizeof(h));
+    h.one = 1;
+    // pageable source: the runtime stages the copy before returning, so the stack object is safe
+    CU(cudaMemcpyAsync(ctx->ctrl, &h, sizeof(h), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->has_state = true;
+    return ECHO_OK;
+}
+
+int echo_set_primitives_host(echo_ctx *ctx, const double *rho, const double *vx, const double *vy, const double *vz,
+                             const double *p, const double *bxf, const double *byf, const double *bzf) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    if (!rho || !vx || !vy || !vz || !p || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
+    const size_t nb = sizeof(double) * ctx->g.N;
+    const double *src[8] = {rho, vx, vy, vz, p, bxf, byf, bzf};
+    double *dst[8];
+    for (int v = 0; v < 5; ++v) dst[v] = ctx->field[F_P + v];       // scratch: the primitive fields
+    for (int d = 0; d < 3; ++d) dst[5 + d] = ctx->field[F_BF + d];  // faces go straight into the state
+    for (int v = 0; v < 8; ++v) CU(cudaMemcpyAsync(dst[v], src[v], nb, cudaMemcpyHostToDevice, ctx->stream));
+    return echo_set_primitives(ctx, dst[0], dst[1], dst[2], dst[3], dst[4], dst[5], dst[6], dst[7]);
+}
+
+int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay, const double *az, double b0x,
+                              double b0y, double b0z, double *bxf, double *byf, double *bzf) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    if (!ax || !ay || !az || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
+    const Grid &g = ctx->g;
+    k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ax, ay, az, bxf, byf, bzf, -1.0, b0x, b0y, b0z);
+    LAUNCH_CHECK("k_curl");
+    return ECHO_OK;
+}
+
+int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
+    const int *active = &ctx->ctrl->active;
+    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    for (int n = 0; n < nsteps; ++n) {
+        k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end);
+        LAUNCH_CHECK("k_begin_step");
+        // stage 1: U1 = U^n + dt L(U^n), dt from the speeds of this very operator (S9)
+        if ((rc = launch_operator(ctx, s0, active, 2))) return rc;
+        if ((rc = launch_update(ctx, s0, 0, 1, 0.0, 1.0, active))) return rc;
+        // stage 2: U2 = 3/4 U^n + 1/4 (U1 + dt L(U1))
+        if ((rc = launch_operator(ctx, s1, active, 0))) return rc;
+        if ((rc = launch_update(ctx, s1, 1, 1, 0.75, 0.25, active))) return rc;
+        // stage 3: U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
+        if ((rc = launch_operator(ctx, s1, active, 0))) return rc;
+        if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, active))) return rc;
+        k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl);
+        LAUNCH_CHECK("k_end_step");
+    }
+    return ECHO_OK;
+}
+
+int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p, double *bxc,
+                        double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!rho || !vx || !vy || !vz || !p || !bxc || !byc || !bzc) return fail(ctx, ECHO_EINVAL, "null array");
+    const Grid &g = ctx->g;
+    Stage st = make_stage(ctx, 0);
+    double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
+    for (int v = 0; v < 5; ++v) st.P[v] = out[v];
+    for (int d = 0; d < 3; ++d) st.Bc[d] = out[5 + d];
+    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, &ctx->ctrl->one);
+    LAUNCH_CHECK("k_prim");
+    double *bf[3] = {bxf, byf, bzf};
+    for (int d = 0; d < 3; ++d)
+        if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
+    return ECHO_OK;
+}
+
+int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p, double *bxc,
+                             double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!rho || !vx || !vy || !vz || !p || !bxc || !byc || !bzc) return fail(ctx, ECHO_EINVAL, "null array");
+    const Grid &g = ctx->g;
+    const size_t nb = sizeof(double) * g.N;
+    Stage st = make_stage(ctx, 0);
+    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, &ctx->ctrl->one);
+    LAUNCH_CHECK("k_prim");
+    double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
+    for (int v = 0; v < 8; ++v) CU(cudaMemcpyAsync(out[v], ctx->field[F_P + v], nb, cudaMemcpyDeviceToHost, ctx->stream));
+    double *bf[3] = {bxf, byf, bzf};
+    for (int d = 0; d < 3; ++d)
+        if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], nb, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return ECHO_OK;
+}
+
+int echo_get_conserved(echo_ctx *ctx, double *D, double *Sx, double *Sy, double *Sz, double *U) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    double *out[5] = {D, Sx, Sy, Sz, U};
+    for (int v = 0; v < 5; ++v) {
+        if (!out[v]) return fail(ctx, ECHO_EINVAL, "null array");
+        CU(cudaMemcpyAsync(out[v], ctx->field[F_U + v], sizeof(double) * ctx->g.N, cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    return ECHO_OK;
+}
+
+int echo_rhs(echo_ctx *ctx, double *const *rhsU, double *const *rhsB, double *const *E, double *amax_host) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    const Grid &g = ctx->g;
+    const size_t nb = sizeof(double) * g.N;
+    const Stage st = make_stage(ctx, 0);
+    CU(cudaMemsetAsync(&ctx->ctrl->amax_bits, 0, sizeof(unsigned long long), ctx->stream));
+    if ((rc = launch_operator(ctx, st, &ctx->ctrl->one, 1))) return rc;
+    if (rhsU)
+        for (int v = 0; v < 5; ++v) CU(cudaMemcpyAsync(rhsU[v], st.R[v], nb, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (E)
+        for (int d = 0; d < 3; ++d) CU(cudaMemcpyAsync(E[d], st.E[d], nb, cudaMemcpyDeviceToDevice, ctx->stream));
+    if (rhsB) {
+        k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], rhsB[0], rhsB[1], rhsB[2],
+                                                               1.0, 0.0, 0.0, 0.0);
+        LAUNCH_CHECK("k_curl");
+    }
+    if (amax_host) {
+        unsigned long long bits = 0;
+        CU(cudaMemcpyAsync(&bits, &ctx->ctrl->amax_bits, sizeof(bits), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        std::memcpy(amax_host, &bits, sizeof(double));
+    }
+    return ECHO_OK;
+}
+
+int echo_con2prim(double gamma, long n, const double *D, const double *Sx, const double *Sy, const double *Sz,
+                  const double *U, const double *Bx, const double *By, const double *Bz, double *rho, double *vx,
+                  double *vy, double *vz, double *p, int *iters, void *cuda_stream) {
+    if (n < 0 || !(gamma > 1.0)) return ECHO_EINVAL;
+    if (n == 0) return ECHO_OK;
+    if (!D || !Sx || !Sy || !Sz || !U || !Bx || !By || !Bz || !rho || !vx || !vy || !vz || !p) return ECHO_EINVAL;
+    const int blocks = (int)std::min<long long>((n + 255) / 256, 148LL * 16);
+    k_c2p_batch<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(gamma, n, D, Sx, Sy, Sz, U, Bx, By, Bz, rho,
+                                                                          vx, vy, vz, p, iters);
+    return cudaGetLastError() == cudaSuccess ? ECHO_OK : ECHO_ECUDA;
+}
+
+int echo_prim2cons(double gamma, long n, const double *rho, const double *vx, const double *vy, const double *vz,
+                   const double *p, const double *Bx, const double *By, const double *Bz, double *D, double *Sx,
+                   double *Sy, double *Sz, double *U, void *cuda_stream) {
+    if (n < 0 || !(gamma > 1.0)) return ECHO_EINVAL;
+    if (n == 0) return ECHO_OK;
+    if (!D || !Sx || !Sy || !Sz || !U || !Bx || !By || !Bz || !rho || !vx || !vy || !vz || !p) return ECHO_EINVAL;
+    const int blocks = (int)std::min<long long>((n + 255) / 256, 148LL * 16);
+    k_p2c_batch<<<blocks, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(gamma / (gamma - 1.0), n, rho, vx, vy, vz, p,
+                                                                          Bx, By, Bz, D, Sx, Sy, Sz, U);
+    return cudaGetLastError() == cudaSuccess ? ECHO_OK : ECHO_ECUDA;
+}
+
+int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    const Grid &g = ctx->g;
+    double *slot = ctx->part + 15 * NPART;   // spare partial row: one double for the max
+    CU(cudaMemsetAsync(slot, 0, sizeof(double), ctx->stream));
+    k_divb<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ctx->field[F_BF], ctx->field[F_BF + 1], ctx->field[F_BF + 2],
+                                                           div_field, slot);
+    LAUNCH_CHECK("k_divb");
+    double m = 0.0;
+    CU(cudaMemcpyAsync(&m, slot, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (max_abs_host) *max_abs_host = m;
+    return ECHO_OK;
+}
+
+int echo_diagnostics(echo_ctx *ctx, double *out) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (!out) return fail(ctx, ECHO_EINVAL, "null output");
+    const Grid &g = ctx->g;
+    for (int m = 0; m < ECHO_NDIAG; ++m) out[m] = 0.0;
+    double *f = ctx->field[F_U];
+    const long long np = ctx->npad;
+    k_sums<<<NPART, 256, 0, ctx->stream>>>(g.N, f, f + np, f + 2 * np, f + 3 * np, f + 4 * np, f + 5 * np, f + 6 * np,
+                                           f + 7 * np, ctx->part);
+    LAUNCH_CHECK("k_sums");
+    Stage st = make_stage(ctx, 0);
+    k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl);
+    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, &ctx->ctrl->one);
+    LAUNCH_CHECK("k_prim");
+    k_extrema<<<NPART, 256, 0, ctx->stream>>>(g.N, st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], ctx->part);
+    LAUNCH_CHECK("k_extrema");
+    double dmax = 0.0;
+    if ((rc = echo_div_b(ctx, nullptr, &dmax))) return rc;   // synchronises
+    std::vector<double> part((size_t)NPART * 11);
+    Ctrl h;
+    CU(cudaMemcpy(part.data(), ctx->part, sizeof(double) * part.size(), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(&h, ctx->ctrl, sizeof(h), cudaMemcpyDeviceToHost));
+    const double vol = g.h[0] * g.h[1] * g.h[2];
+    out[0] = h.t; out[1] = h.dt_last; out[2] = (double)h.steps; out[3] = h.amax;
+    for (int v = 0; v < 8; ++v) {
+        long double s = 0.0L;
+        for (int b = 0; b < NPART; ++b) s += part[(size_t)v * NPART + b];
+        out[4 + v] = (double)(s * vol);
+    }
+    out[12] = dmax;
+    double v2m = 0.0, rmin = INFINITY, pmin = INFINITY;
+    for (int b = 0; b < NPART; ++b) {
+        if ((long long)b * ((g.N + NPART - 1) / NPART) >= g.N) break;   // empty chunks hold no data
+        v2m = std::fmax(v2m, part[8 * (size_t)NPART + b]);
+        rmin = std::fmin(rmin, part[9 * (size_t)NPART + b]);
+        pmin = std::fmin(pmin, part[10 * (size_t)NPART + b]);
+    }
+    out[13] = 1.0 / std::sqrt(1.0 - v2m);
+    out[14] = rmin;
+    out[15] = pmin;
+    out[16] = (double)h.c2p_maxit;
+    out[17] = h.c2p_calls ? (double)h.c2p_sumit / (double)h.c2p_calls : 0.0;
+    out[18] = (double)h.c2p_fail_total;
+    return h.c2p_fail_total ? fail(ctx, ECHO_EC2P, "con2prim failed in at least one cell") : ECHO_OK;
+}
+
+}  // extern "C"

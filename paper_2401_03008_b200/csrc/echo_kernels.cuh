@@ -1,0 +1,468 @@
+// echo_kernels.cuh — the kernels of one Runge-Kutta sub-step, sm_100a, FP64.
+//   k_prim      point 1: INT of the staggered B + con2prim                    (a1, a2)
+//   k_flux<D>   points 2+3: REC -> L/R -> HLL flux -> DER + divergence  (a3, a4, a8)
+//   k_uct       point 4: UCT edge EMFs                                        (a5)
+//   k_update    point 4b + 5 (eq.(10)): curl of DER(E) + RK combination (a6, a7)
+// plus the small control kernels that keep t, dt and a_max on the device.
+#pragma once
+#include "echo_math.cuh"
+#include "echo_types.cuh"
+
+namespace echo {
+
+// periodic wrap; the fast path is a range check, the modulo only runs next to the seams
+__device__ __forceinline__ int wrapi(int a, int n) {
+    if ((unsigned)a >= (unsigned)n) {
+        a %= n;
+        if (a < 0) a += n;
+    }
+    return a;
+}
+
+__device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double v) {
+    // bit patterns of non-negative doubles order like unsigned integers; max is exact and
+    // order-independent, so the reduction is deterministic (P:L198 reduce(max:amax))
+    atomicMax(addr, (unsigned long long)__double_as_longlong(v));
+}
+
+// ------------------------------------------------------------------ control kernels (1 thread)
+__global__ void k_begin_step(Ctrl *c, double t_end) {
+    c->t_end = t_end;
+    c->active = (c->t < t_end) ? 1 : 0;
+    c->amax_bits = 0ull;
+}
+__global__ void k_set_dt(Ctrl *c, double cfl_hmin) {
+    if (!c->active) return;
+    const double amax = __longlong_as_double((long long)c->amax_bits);
+    double dt = cfl_hmin / amax;
+    if (c->t + dt > c->t_end) dt = c->t_end - c->t;
+    c->amax = amax;
+    c->dt = dt;
+}
+__global__ void k_end_step(Ctrl *c) {
+    if (!c->active) return;
+    c->t += c->dt;
+    c->dt_last = c->dt;
+    c->steps += 1;
+}
+__global__ void k_c2p_stats_reset(Ctrl *c) {
+    c->c2p_sumit = 0ull; c->c2p_calls = 0ull; c->c2p_fail = 0ull; c->c2p_maxit = 0;
+}
+
+// ------------------------------------------------------------------ point 1: INT + con2prim
+// One thread per cell, block (64,4,1).  Face B comes in through L1/L2 with 6-point stencils.
+__global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, const int *active) {
+    if (!*active) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    int it = 0;
+    const bool in = (i < g.n[0]) && (j < g.n[1]);
+    if (in) {
+        const int c3[3] = {i, j, k};
+        const long long c = i + g.s[1] * j + g.s[2] * k;
+        double B[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const long long base = c - g.s[d] * c3[d];
+            double b[6];
+#pragma unroll
+            for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]));
+            B[d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
+        }
+        const double u[5] = {st.U[0][c], st.U[1][c], st.U[2][c], st.U[3][c], st.U[4][c]};
+        double q[5];
+        it = con2prim(gam, u, B, q);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) st.P[v][c] = q[v];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) st.Bc[d][c] = B[d];
+    }
+    // statistics: warp reduction, one atomic per warp
+    const int ai = it < 0 ? -it : it;
+    int sum = ai, mx = ai, fail = it < 0 ? 1 : 0, calls = in ? 1 : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        fail += __shfl_xor_sync(0xffffffffu, fail, o);
+        calls += __shfl_xor_sync(0xffffffffu, calls, o);
+    }
+    if (((threadIdx.y * blockDim.x + threadIdx.x) & 31) == 0) {
+        atomicAdd(&ctrl->c2p_sumit, (unsigned long long)sum);
+        atomicAdd(&ctrl->c2p_calls, (unsigned long long)calls);
+        atomicMax(&ctrl->c2p_maxit, mx);
+        if (fail) {
+            atomicAdd(&ctrl->c2p_fail, (unsigned long long)fail);
+            atomicAdd(&ctrl->c2p_fail_total, (unsigned long long)fail);
+        }
+    }
+}
+
+// set_primitives: INT + prim2cons.  prim[0..4] = rho, vx, vy, vz, p; faces in Bf.
+__global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const double *vx, const double *vy,
+                                              const double *vz, const double *p, const double *bf0,
+                                              const double *bf1, const double *bf2, double *U0, double *U1,
+                                              double *U2, double *U3, double *U4, double gg) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= g.n[0] || j >= g.n[1]) return;
+    const int c3[3] = {i, j, k};
+    const long long c = i + g.s[1] * j + g.s[2] * k;
+    const double *bf[3] = {bf0, bf1, bf2};
+    double q[8] = {rho[c], vx[c], vy[c], vz[c], p[c], 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const long long base = c - g.s[d] * c3[d];
+        double b[6];
+#pragma unroll
+        for (int m = 0; m < 6; ++m) b[m] = __ldg(bf[d] + base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]));
+        q[5 + d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
+    }
+    double u[5];
+    prim2cons(gg, q, u);
+    U0[c] = u[0]; U1[c] = u[1]; U2[c] = u[2]; U3[c] = u[3]; U4[c] = u[4];
+}
+
+// ------------------------------------------------------------------ points 2+3: fused flux sweep
+// Direction D.  A block owns a tile of L cells along D times T cells along the contiguous
+// transverse axis TD (y for the x-sweep, x otherwise) at one coordinate of the remaining axis.
+// Phase 1: the L+5 face fluxes F_{m0-3 .. m0+L+1} (5 components) go to shared memory; faces
+// m0..m0+L-1 also store a+, a-, vbar and feed the a_max reduction.
+// Phase 2: rhs -= (F^_{i+1/2} - F^_{i-1/2})/h_D from shared memory (DER).  The 5 halo
+// faces are recomputed by the neighbouring tile with the same instructions on the same inputs,
+// hence bit-identically: conservation stays at round-off.
+struct FluxTile { int L, T, tilesD, tilesT; };
+
+template <int D, int NT>
+__global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, FluxTile tl, double gam, double gg, Ctrl *ctrl,
+                                             const int *active, int want_amax) {
+    if (!*active) return;
+    constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
+    constexpr int OD = 3 - D - TD;            // remaining axis
+    constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
+    extern __shared__ double sF[];
+    const int L = tl.L, T = tl.T, LA = L + 5;
+    const int tileT = blockIdx.x, tileD = blockIdx.y;
+    const int cO = blockIdx.z;
+    const int m0 = tileD * L;
+    const int t0 = tileT * T;
+    const int nD = g.n[D], nT = g.n[TD];
+    const int Lv = min(L, nD - m0);           // valid cells of this tile along D
+    const long long sD = g.s[D], sT = g.s[TD];
+    const long long baseO = g.s[OD] * cO;
+    const int nface = LA * T;
+    double amax = 0.0;
+
+    for (int f = threadIdx.x; f < nface; f += NT) {
+        int a, b;
+        if (D == 0) { a = f % LA; b = f / LA; } else { b = f % T; a = f / T; }
+        const int cT = t0 + b;
+        if (cT >= nT || a >= Lv + 5) continue;
+        const int m = m0 - 3 + a;             // face m sits between cells m and m+1
+        long long idx[6];
+#pragma unroll
+        for (int s = 0; s < 6; ++s) idx[s] = baseO + sT * cT + sD * wrapi(m - 2 + s, nD);
+        double qL[8], qR[8];
+        {
+            const double *rec[7] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2]};
+            const int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+#pragma unroll
+            for (int v = 0; v < 7; ++v) {
+                double s[6];
+#pragma unroll
+                for (int k = 0; k < 6; ++k) s[k] = __ldg(rec[v] + idx[k]);
+                qL[slot[v]] = mp5(s[0], s[1], s[2], s[3], s[4]);
+                qR[slot[v]] = mp5(s[5], s[4], s[3], s[2], s[1]);
+            }
+        }
+        qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + idx[2]);   // the normal B is the staggered value
+        double F[5], ap, am, vb1, vb2;
+        hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
+        const int so = (D == 0) ? (b * LA + a) : (a * T + b);
+#pragma unroll
+        for (int c = 0; c < 5; ++c) sF[c * nface + so] = F[c];
+        if (a >= 3 && a < Lv + 3) {
+            const long long o = idx[2];
+            st.ap[D][o] = ap;
+            st.am[D][o] = am;
+            st.vb[D][0][o] = vb1;
+            st.vb[D][1][o] = vb2;
+            amax = fmax(amax, fmax(ap, am));
+        }
+    }
+    __syncthreads();
+
+    const double rh = g.rh[D];
+    const int ncell = L * T;
+    for (int e = threadIdx.x; e < ncell; e += NT) {
+        int a, b;
+        if (D == 0) { a = e % L; b = e / L; } else { b = e % T; a = e / T; }
+        const int cT = t0 + b;
+        if (cT >= nT || a >= Lv) continue;
+        const long long o = baseO + sT * cT + sD * (m0 + a);
+        const int step = (D == 0) ? 1 : T;
+        const int so = (D == 0) ? (b * LA + a) : (a * T + b);
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+            const double *F = sF + c * nface + so;
+            const double r = -rh * der_diff(F[0], F[step], F[2 * step], F[3 * step], F[4 * step], F[5 * step]);
+            if (D == 0) st.R[c][o] = r; else st.R[c][o] += r;
+        }
+    }
+
+    if (want_amax) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        __shared__ double wmax[NT / 32];
+        if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = amax;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double m = wmax[0];
+#pragma unroll
+            for (int w = 1; w < NT / 32; ++w) m = fmax(m, wmax[w]);
+            atomic_max_nonneg(&ctrl->amax_bits, m);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ point 4: UCT edge EMFs (O7)
+// One thread per cell computes the three edge EMFs attached to it.  For the k-edge, with
+// i = (k+1)%3, j = (k+2)%3:   E_k = -HLL_i[ vbar_i B_j ] + HLL_j[ vbar_j B_i ]
+// where (vbar_i saved at j-faces, staggered B_j) are MP5-reconstructed along i and the edge speeds
+// are the max of the saved face speeds over the two faces adjacent to the edge.
+template <int K>
+__device__ __forceinline__ double uct_edge(const Stage &st, const long long (*ix)[6], long long c) {
+    constexpr int I = (K + 1) % 3, J = (K + 2) % 3;
+    // slots: direction J saves vbar_{(J+1)%3} = vbar_K in [0], vbar_{(J+2)%3} = vbar_I in [1];
+    //        direction I saves vbar_{(I+1)%3} = vbar_J in [0]
+    const double *vi = st.vb[J][1], *vj = st.vb[I][0];
+    const double *Bi = st.Bf[I], *Bj = st.Bf[J];
+    double s[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) s[m] = __ldg(vi + ix[I][m]);
+    const double viL = mp5(s[0], s[1], s[2], s[3], s[4]), viR = mp5(s[5], s[4], s[3], s[2], s[1]);
+#pragma unroll
+    for (int m = 0; m < 6; ++m) s[m] = __ldg(Bj + ix[I][m]);
+    const double BjL = mp5(s[0], s[1], s[2], s[3], s[4]), BjR = mp5(s[5], s[4], s[3], s[2], s[1]);
+#pragma unroll
+    for (int m = 0; m < 6; ++m) s[m] = __ldg(vj + ix[J][m]);
+    const double vjL = mp5(s[0], s[1], s[2], s[3], s[4]), vjR = mp5(s[5], s[4], s[3], s[2], s[1]);
+#pragma unroll
+    for (int m = 0; m < 6; ++m) s[m] = __ldg(Bi + ix[J][m]);
+    const double BiL = mp5(s[0], s[1], s[2], s[3], s[4]), BiR = mp5(s[5], s[4], s[3], s[2], s[1]);
+    const long long cj = ix[J][3], ci = ix[I][3];   // neighbours +1 along j and along i
+    const double aip = fmax(__ldg(st.ap[I] + c), __ldg(st.ap[I] + cj));
+    const double aim = fmax(__ldg(st.am[I] + c), __ldg(st.am[I] + cj));
+    const double ajp = fmax(__ldg(st.ap[J] + c), __ldg(st.ap[J] + ci));
+    const double ajm = fmax(__ldg(st.am[J] + c), __ldg(st.am[J] + ci));
+    return -(aip * viL * BjL + aim * viR * BjR - aip * aim * (BjR - BjL)) / (aip + aim) +
+           (ajp * vjL * BiL + ajm * vjR * BiR - ajp * ajm * (BiR - BiL)) / (ajp + ajm);
+}
+
+__global__ void __launch_bounds__(256) k_uct(Grid g, Stage st, const int *active) {
+    if (!*active) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= g.n[0] || j >= g.n[1]) return;
+    const int c3[3] = {i, j, k};
+    const long long c = i + g.s[1] * j + g.s[2] * k;
+    long long ix[3][6];   // cells c-2 .. c+3 along each axis
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const long long base = c - g.s[d] * c3[d];
+#pragma unroll
+        for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 2, g.n[d]);
+    }
+    st.E[0][c] = uct_edge<0>(st, ix, c);
+    st.E[1][c] = uct_edge<1>(st, ix, c);
+    st.E[2][c] = uct_edge<2>(st, ix, c);
+}
+
+// ------------------------------------------------------------------ points 4b + 5: curl + RK update
+// rhs of the staggered B (O8, eq.(10)): dB_i/dt = -[ D_j(DER_j E_k) - D_k(DER_k E_j) ],
+// then for all 8 evolved fields  out = c0*base + c1*(cur + dt*rhs)  (O9).
+// dt is read from the device control block (a8: no host round trip).
+template <int I>
+__device__ __forceinline__ double curl_comp(const Grid &g, const double *const E[3], const long long (*ix)[6]) {
+    constexpr int J = (I + 1) % 3, K = (I + 2) % 3;
+    double a[6], b[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) { a[m] = __ldg(E[K] + ix[J][m]); b[m] = __ldg(E[J] + ix[K][m]); }
+    return -(g.rh[J] * der_diff(a[0], a[1], a[2], a[3], a[4], a[5]) -
+             g.rh[K] * der_diff(b[0], b[1], b[2], b[3], b[4], b[5]));
+}
+
+__global__ void __launch_bounds__(256) k_update(Grid g, const double *E0, const double *E1, const double *E2,
+                                                const double *R0, const double *R1, const double *R2,
+                                                const double *R3, const double *R4, Update up, const Ctrl *ctrl,
+                                                const int *active) {
+    if (!*active) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= g.n[0] || j >= g.n[1]) return;
+    const int c3[3] = {i, j, k};
+    const long long c = i + g.s[1] * j + g.s[2] * k;
+    const double dt = ctrl->dt;
+    long long ix[3][6];   // cells c-3 .. c+2 along each axis (faces/edges i-5/2 .. i+5/2 of the difference)
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const long long base = c - g.s[d] * c3[d];
+#pragma unroll
+        for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]);
+    }
+    const double *const E[3] = {E0, E1, E2};
+    double r[8] = {R0[c], R1[c], R2[c], R3[c], R4[c], 0.0, 0.0, 0.0};
+    r[5] = curl_comp<0>(g, E, ix);
+    r[6] = curl_comp<1>(g, E, ix);
+    r[7] = curl_comp<2>(g, E, ix);
+#pragma unroll
+    for (int v = 0; v < 8; ++v) {
+        const double cur = up.cur[v][c];
+        const double adv = cur + dt * r[v];
+        up.out[v][c] = (up.c0 == 0.0) ? adv : up.c0 * up.base[v][c] + up.c1 * adv;
+    }
+}
+
+// rhs of B alone (echo_rhs) and B = curl A (echo_faces_from_potential, sign = +1, S11)
+__global__ void __launch_bounds__(256) k_curl(Grid g, const double *E0, const double *E1, const double *E2,
+                                              double *o0, double *o1, double *o2, double sign, double b0x,
+                                              double b0y, double b0z) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= g.n[0] || j >= g.n[1]) return;
+    const int c3[3] = {i, j, k};
+    const long long c = i + g.s[1] * j + g.s[2] * k;
+    long long ix[3][6];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const long long base = c - g.s[d] * c3[d];
+#pragma unroll
+        for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]);
+    }
+    const double *const E[3] = {E0, E1, E2};
+    // curl_comp returns -(curl E)_i; sign = +1 gives rhs_B = -curl E, sign = -1 gives +curl A
+    o0[c] = sign * curl_comp<0>(g, E, ix) + b0x;
+    o1[c] = sign * curl_comp<1>(g, E, ix) + b0y;
+    o2[c] = sign * curl_comp<2>(g, E, ix) + b0z;
+}
+
+// ------------------------------------------------------------------ S10: high-order div B
+__global__ void __launch_bounds__(256) k_divb(Grid g, const double *B0, const double *B1, const double *B2,
+                                              double *div, double *blockmax) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    double v = 0.0;
+    if (i < g.n[0] && j < g.n[1]) {
+        const int c3[3] = {i, j, k};
+        const long long c = i + g.s[1] * j + g.s[2] * k;
+        const double *B[3] = {B0, B1, B2};
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const long long base = c - g.s[d] * c3[d];
+            double f[6];
+#pragma unroll
+            for (int m = 0; m < 6; ++m) f[m] = __ldg(B[d] + base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]));
+            v += g.rh[d] * der_diff(f[0], f[1], f[2], f[3], f[4], f[5]);
+        }
+        if (div) div[c] = v;
+        v = fabs(v);
+    }
+    __shared__ double sm[256];
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    sm[tid] = v;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (tid < s) sm[tid] = fmax(sm[tid], sm[tid + s]);
+        __syncthreads();
+    }
+    if (tid == 0) atomic_max_nonneg((unsigned long long *)blockmax, sm[0]);
+}
+
+// ------------------------------------------------------------------ deterministic reductions
+// NPART contiguous chunks; each block sums its chunk with a fixed tree, the host adds the NPART
+// partials in extended precision.  rows 0..7: sums of the 8 evolved fields.
+__global__ void __launch_bounds__(256) k_sums(long long N, const double *f0, const double *f1, const double *f2,
+                                              const double *f3, const double *f4, const double *f5,
+                                              const double *f6, const double *f7, double *part) {
+    const double *f[8] = {f0, f1, f2, f3, f4, f5, f6, f7};
+    const long long chunk = (N + NPART - 1) / NPART;
+    const long long lo = chunk * blockIdx.x, hi = min(N, lo + chunk);
+    __shared__ double sm[256];
+    for (int v = 0; v < 8; ++v) {
+        double s = 0.0;
+        for (long long c = lo + threadIdx.x; c < hi; c += 256) s += f[v][c];
+        sm[threadIdx.x] = s;
+        __syncthreads();
+        for (int w = 128; w > 0; w >>= 1) {
+            if (threadIdx.x < w) sm[threadIdx.x] += sm[threadIdx.x + w];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) part[v * NPART + blockIdx.x] = sm[0];
+        __syncthreads();
+    }
+}
+
+// rows 8..10: max v^2, min rho, min p per chunk (of the primitives of the last k_prim pass)
+__global__ void __launch_bounds__(256) k_extrema(long long N, const double *rho, const double *vx, const double *vy,
+                                                 const double *vz, const double *p, double *part) {
+    const long long chunk = (N + NPART - 1) / NPART;
+    const long long lo = chunk * blockIdx.x, hi = min(N, lo + chunk);
+    __shared__ double s0[256], s1[256], s2[256];
+    double v2m = 0.0, rmin = INFINITY, pmin = INFINITY;
+    for (long long c = lo + threadIdx.x; c < hi; c += 256) {
+        v2m = fmax(v2m, vx[c] * vx[c] + vy[c] * vy[c] + vz[c] * vz[c]);
+        rmin = fmin(rmin, rho[c]);
+        pmin = fmin(pmin, p[c]);
+    }
+    s0[threadIdx.x] = v2m; s1[threadIdx.x] = rmin; s2[threadIdx.x] = pmin;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (threadIdx.x < w) {
+            s0[threadIdx.x] = fmax(s0[threadIdx.x], s0[threadIdx.x + w]);
+            s1[threadIdx.x] = fmin(s1[threadIdx.x], s1[threadIdx.x + w]);
+            s2[threadIdx.x] = fmin(s2[threadIdx.x], s2[threadIdx.x + w]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        part[8 * NPART + blockIdx.x] = s0[0];
+        part[9 * NPART + blockIdx.x] = s1[0];
+        part[10 * NPART + blockIdx.x] = s2[0];
+    }
+}
+
+// ------------------------------------------------------------------ stateless batched point maps
+__global__ void __launch_bounds__(256) k_c2p_batch(double gam, long long n, const double *D, const double *Sx,
+                                                   const double *Sy, const double *Sz, const double *U,
+                                                   const double *Bx, const double *By, const double *Bz,
+                                                   double *rho, double *vx, double *vy, double *vz, double *p,
+                                                   int *iters) {
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < n; c += (long long)gridDim.x * blockDim.x) {
+        const double u[5] = {D[c], Sx[c], Sy[c], Sz[c], U[c]};
+        const double B[3] = {Bx[c], By[c], Bz[c]};
+        double q[5];
+        const int it = con2prim(gam, u, B, q);
+        rho[c] = q[0]; vx[c] = q[1]; vy[c] = q[2]; vz[c] = q[3]; p[c] = q[4];
+        if (iters) iters[c] = it;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_p2c_batch(double gg, long long n, const double *rho, const double *vx,
+                                                   const double *vy, const double *vz, const double *p,
+                                                   const double *Bx, const double *By, const double *Bz, double *D,
+                                                   double *Sx, double *Sy, double *Sz, double *U) {
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < n; c += (long long)gridDim.x * blockDim.x) {
+        const double q[8] = {rho[c], vx[c], vy[c], vz[c], p[c], Bx[c], By[c], Bz[c]};
+        double u[5];
+        prim2cons(gg, q, u);
+        D[c] = u[0]; Sx[c] = u[1]; Sy[c] = u[2]; Sz[c] = u[3]; U[c] = u[4];
+    }
+}
+
+}  // namespace echo

@@ -1,0 +1,213 @@
+// echo_math.cuh — per-point device functions of the ECHO RMHD step (FP64, sm_100a).
+// Stencil operators INT / DER / REC (coefficients: DESIGN.md O1, O3, O6), point
+// physics (definitions, eq.(6), eq.(8)), fast speeds (O4), HLL (O5) and
+// the Newton conservative->primitive inversion (O2).  Written from the paper / DESIGN.md;
+// shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace echo {
+
+// ---------------------------------------------------------------- stencils
+// O1 — INT: 6-point Lagrange interpolation of staggered point values to the midpoint.
+__device__ __forceinline__ double int6(double b0, double b1, double b2, double b3, double b4, double b5) {
+    return (150.0 / 256.0) * (b2 + b3) - (25.0 / 256.0) * (b1 + b4) + (3.0 / 256.0) * (b0 + b5);
+}
+
+// O6 — DER then two-point difference, folded into one antisymmetric 6-point stencil:
+// F^_{i+1/2} - F^_{i-1/2} with F^ = d0 F + d2 (F_-1 + F_+1) + d4 (F_-2 + F_+2),
+// (d0,d2,d4) = (1067/960, -29/480, 3/640)  =>  (75/64, -25/384, 3/640) on the three differences.
+// f0..f5 = F at faces i-5/2, i-3/2, i-1/2, i+1/2, i+3/2, i+5/2.
+__device__ __forceinline__ double der_diff(double f0, double f1, double f2, double f3, double f4, double f5) {
+    return (75.0 / 64.0) * (f3 - f2) + ((-25.0 / 384.0) * (f4 - f1) + (3.0 / 640.0) * (f5 - f0));
+}
+
+__device__ __forceinline__ double minmod2(double a, double b) {
+    // same sign: the one of smaller magnitude; else 0
+    const double m = fmin(fabs(a), fabs(b));
+    return (a * b > 0.0) ? copysign(m, a) : 0.0;
+}
+__device__ __forceinline__ double minmod4(double a, double b, double c, double d) {
+    const bool pos = (a > 0.0) & (b > 0.0) & (c > 0.0) & (d > 0.0);
+    const bool neg = (a < 0.0) & (b < 0.0) & (c < 0.0) & (d < 0.0);
+    const double mn = fmin(fmin(a, b), fmin(c, d));
+    const double mx = fmax(fmax(a, b), fmax(c, d));
+    return pos ? mn : (neg ? mx : 0.0);
+}
+
+// O3 — REC: MP5 (Suresh & Huynh 1997) on POINT values.  Left-biased value at i+1/2
+// from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (S2).
+__device__ __noinline__ double mp5_limited(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
+    const double alpha = 4.0;
+    const double dm1 = vm2 - 2.0 * vm1 + v0;
+    const double d0 = vm1 - 2.0 * v0 + vp1;
+    const double dp1 = v0 - 2.0 * vp1 + vp2;
+    const double dm4p = minmod4(4.0 * d0 - dp1, 4.0 * dp1 - d0, d0, dp1);
+    const double dm4m = minmod4(4.0 * dm1 - d0, 4.0 * d0 - dm1, dm1, d0);
+    const double vul = v0 + alpha * (v0 - vm1);
+    const double vav = 0.5 * (v0 + vp1);
+    const double vmd = vav - 0.5 * dm4p;
+    const double vlc = v0 + 0.5 * (v0 - vm1) + (4.0 / 3.0) * dm4m;
+    const double vmin = fmax(fmin(v0, fmin(vp1, vmd)), fmin(v0, fmin(vul, vlc)));
+    const double vmax = fmin(fmax(v0, fmax(vp1, vmd)), fmax(v0, fmax(vul, vlc)));
+    return vor + minmod2(vmin - vor, vmax - vor);
+}
+
+__device__ __forceinline__ double mp5(double vm2, double vm1, double v0, double vp1, double vp2) {
+    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
+                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
+    const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
+    if ((vor - v0) * (vor - vmp) <= 1e-10) return vor;
+    return mp5_limited(vm2, vm1, v0, vp1, vp2, vor);
+}
+
+// ---------------------------------------------------------------- point physics
+// q[8] = (rho, vx, vy, vz, p, Bx, By, Bz); u[5] = (D, Sx, Sy, Sz, U).  gg = gamma/(gamma-1).
+// Identities used (E = -v x B): E x B = B^2 v - (v.B) B, E^2 = v^2 B^2 - (v.B)^2.
+__device__ __forceinline__ void prim2cons(double gg, const double q[8], double u[5]) {
+    const double v2 = q[1] * q[1] + q[2] * q[2] + q[3] * q[3];
+    const double B2 = q[5] * q[5] + q[6] * q[6] + q[7] * q[7];
+    const double vB = q[1] * q[5] + q[2] * q[6] + q[3] * q[7];
+    const double W = rsqrt(1.0 - v2);
+    const double y = (q[0] + gg * q[4]) * (W * W);
+    const double yb = y + B2;
+    u[0] = q[0] * W;
+    u[1] = yb * q[1] - vB * q[5];
+    u[2] = yb * q[2] - vB * q[6];
+    u[3] = yb * q[3] - vB * q[7];
+    u[4] = y - q[4] + 0.5 * ((v2 * B2 - vB * vB) + B2);
+}
+
+// One side of a D-face: conserved state u, physical flux f (eq.(8)), fast speeds lp, lm (O4).
+template <int D>
+__device__ __forceinline__ void side_state(double gam, double gg, const double q[8], double u[5], double f[5],
+                                           double &lp, double &lm) {
+    const double rho = q[0], p = q[4];
+    const double v[3] = {q[1], q[2], q[3]};
+    const double B[3] = {q[5], q[6], q[7]};
+    const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    const double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+    const double vB = v[0] * B[0] + v[1] * B[1] + v[2] * B[2];
+    const double omv2 = 1.0 - v2;
+    const double W = rsqrt(omv2);
+    const double rhoh = rho + gg * p;
+    const double y = rhoh * (W * W);
+    const double yb = y + B2;
+    const double E2 = v2 * B2 - vB * vB;
+    const double ptot = p + 0.5 * (E2 + B2);
+    // E = -v x B
+    const double E[3] = {-(v[1] * B[2] - v[2] * B[1]), -(v[2] * B[0] - v[0] * B[2]), -(v[0] * B[1] - v[1] * B[0])};
+    u[0] = rho * W;
+    u[1] = yb * v[0] - vB * B[0];
+    u[2] = yb * v[1] - vB * B[1];
+    u[3] = yb * v[2] - vB * B[2];
+    u[4] = y - p + 0.5 * (E2 + B2);
+    const double yvd = y * v[D];
+    f[0] = u[0] * v[D];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) f[1 + a] = yvd * v[a] - E[a] * E[D] - B[a] * B[D] + (a == D ? ptot : 0.0);
+    f[4] = u[1 + D];
+    // O4: a^2 = cs^2 + ca^2 - cs^2 ca^2, cs^2 = gamma p/(rho h), ca^2 = b^2/(rho h + b^2)
+    const double b2 = B2 * omv2 + vB * vB;
+    const double w = rhoh + b2;
+    const double r = 1.0 / (rhoh * w);
+    const double cs2 = gam * p * w * r;
+    const double ca2 = b2 * rhoh * r;
+    const double a2 = cs2 + ca2 - cs2 * ca2;
+    const double oma2 = 1.0 - a2;
+    const double den = 1.0 - v2 * a2;
+    const double vd = v[D];
+    const double root = sqrt(a2 * omv2 * (den - oma2 * vd * vd));
+    const double rden = 1.0 / den;
+    lp = (oma2 * vd + root) * rden;
+    lm = (oma2 * vd - root) * rden;
+}
+
+// O5 — two-state HLL flux at a D-face; also the stored UCT pieces:
+// ap, am and the upwind-averaged transverse velocities vb1 = vbar_{(D+1)%3}, vb2 = vbar_{(D+2)%3}.
+template <int D>
+__device__ __forceinline__ void hll_face(double gam, double gg, const double qL[8], const double qR[8], double F[5],
+                                         double &ap, double &am, double &vb1, double &vb2) {
+    double uL[5], fL[5], uR[5], fR[5], lpL, lmL, lpR, lmR;
+    side_state<D>(gam, gg, qL, uL, fL, lpL, lmL);
+    side_state<D>(gam, gg, qR, uR, fR, lpR, lmR);
+    ap = fmax(0.0, fmax(lpL, lpR));
+    am = fmax(0.0, fmax(-lmL, -lmR));
+    const double inv = 1.0 / (ap + am);
+    const double wl = ap * inv, wr = am * inv, wd = ap * am * inv;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) F[c] = wl * fL[c] + wr * fR[c] - wd * (uR[c] - uL[c]);
+    constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
+    vb1 = wl * qL[1 + t1] + wr * qR[1 + t1];
+    vb2 = wl * qL[1 + t2] + wr * qR[1 + t2];
+}
+
+// ---------------------------------------------------------------- O2: con2prim
+// Newton on y = rho h W^2 from the upper bound y0 = gamma (U - B^2/2); safeguard and stopping
+// rule as in DESIGN.md O2.  Returns the number of Newton updates (>=1) or -(count) on failure.
+struct C2PEval { double x, p, f, df; };
+
+__device__ __forceinline__ bool c2p_eval(double g1, double D, double S2, double B2, double T, double U, double y,
+                                         C2PEval &a) {
+    if (!(y > 0.0) || !isfinite(y)) return false;
+    const double yb = y + B2;
+    const double y2 = y * y, yb2 = yb * yb;
+    const double r = 1.0 / (y2 * y * yb2 * yb);   // 1/(y^3 (y+B^2)^3)
+    const double x = (S2 * y2 + T * (2.0 * y + B2)) * (y * yb) * r;
+    if (!(x < 1.0) || !(x >= 0.0)) return false;
+    const double omx = 1.0 - x;
+    const double sq = sqrt(omx);
+    const double xp = -2.0 * (S2 * y2 * y + T * (3.0 * y2 + 3.0 * y * B2 + B2 * B2)) * r;
+    const double Ty3 = T * (yb2 * yb) * r;        // T / y^3
+    a.x = x;
+    a.p = g1 * (y * omx - D * sq);
+    a.f = y - a.p + 0.5 * (1.0 + x) * B2 - 0.5 * Ty3 * y - U;
+    a.df = 1.0 - g1 * omx - g1 * (-y + 0.5 * D / sq) * xp + 0.5 * B2 * xp + Ty3;
+    return true;
+}
+
+__device__ __forceinline__ int con2prim(double gam, const double u[5], const double B[3], double q[5]) {
+    const double tol = 1e-12;
+    const int maxit = 30;
+    const double g1 = (gam - 1.0) / gam;
+    const double D = u[0], U = u[4];
+    const double S2 = u[1] * u[1] + u[2] * u[2] + u[3] * u[3];
+    const double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+    const double SB = u[1] * B[0] + u[2] * B[1] + u[3] * B[2];
+    const double T = SB * SB;
+    double y = gam * (U - 0.5 * B2);
+    double ylast = y;
+    C2PEval a;
+    int it = 0;
+    bool conv = false;
+    while (it < maxit) {
+        if (!c2p_eval(g1, D, S2, B2, T, U, y, a)) {
+            if (it == 0) break;
+            ++it;
+            y = 0.5 * (y + ylast);
+            if (!isfinite(y)) break;
+            continue;
+        }
+        ylast = y;
+        const double dy = -a.f / a.df;
+        y = y + dy;
+        ++it;
+        if (fabs(dy) <= tol * fabs(y)) { conv = true; break; }
+    }
+    if (!conv || !c2p_eval(g1, D, S2, B2, T, U, y, a)) {
+        const double nan = __longlong_as_double(0x7ff8000000000000LL);
+        q[0] = q[1] = q[2] = q[3] = q[4] = nan;
+        return -(it > 0 ? it : 1);
+    }
+    q[0] = D * sqrt(1.0 - a.x);
+    q[4] = a.p;
+    const double ryb = 1.0 / (y + B2);
+    const double sby = SB / y;
+    q[1] = (u[1] + sby * B[0]) * ryb;
+    q[2] = (u[2] + sby * B[1]) * ryb;
+    q[3] = (u[3] + sby * B[2]) * ryb;
+    return it;
+}
+
+}  // namespace echo

@@ -1,0 +1,56 @@
+// echo_types.cuh — plain structs shared by the kernels and the C-ABI layer (device + host).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace echo {
+
+// Grid geometry: unit periodic box, h_d = 1/n_d, x fastest.
+struct Grid {
+    int n[3];
+    long long s[3];   // linear strides: 1, nx, nx*ny
+    long long N;
+    double h[3], rh[3];   // spacing and its reciprocal (n_d exactly)
+};
+
+// Device control block (first bytes of the workspace).  Everything echo_step needs between
+// kernels lives here so that no host synchronisation is needed inside a step.
+struct Ctrl {
+    double t, dt, dt_last, t_end;
+    double amax;                       // last stage-1 maximum characteristic speed (a8)
+    unsigned long long amax_bits;      // running max of non-negative doubles, as their bit pattern
+    long long steps;
+    int active;                        // 0 once t >= t_end: every kernel of the step returns at once
+    int one;                           // constant 1 (the "always active" flag)
+    // con2prim statistics: of the most recent full pass, and failures since set_primitives
+    unsigned long long c2p_sumit, c2p_calls, c2p_fail, c2p_fail_total;
+    int c2p_maxit;
+    int pad_;
+};
+
+constexpr int NFIELD = 44;         // U[5] Bf[3] | U0[5] Bf0[3] | P[5] Bc[3] | R[5] | ap[3] am[3] vb[6] | E[3]
+constexpr int NPART = 1024;        // chunks of the deterministic reductions
+constexpr int NPARTF = 16;         // partial rows (8 sums + spare)
+constexpr size_t CTRL_BYTES = 4096;
+constexpr size_t PART_BYTES = sizeof(double) * NPART * NPARTF;
+
+// Pointers of one stage, passed by value to the kernels.
+struct Stage {
+    const double *U[5];    // conserved state the operator L is applied to
+    const double *Bf[3];   // staggered B of that state
+    double *P[5];          // primitives rho, vx, vy, vz, p
+    double *Bc[3];         // centred B (INT of the faces)
+    double *R[5];          // rhs of the 5 conserved cell fields
+    double *ap[3], *am[3]; // a+ and a- saved at the d-faces
+    double *vb[3][2];      // vbar_{(d+1)%3}, vbar_{(d+2)%3} saved at the d-faces
+    double *E[3];          // edge EMFs
+};
+
+// RK combination  out = c0 * base + c1 * (cur + dt * rhs)   (O9)
+struct Update {
+    const double *base[8];   // U^n, Bf^n
+    const double *cur[8];    // state the stage started from
+    double *out[8];
+    double c0, c1;
+};
+
+}  // namespace echo
