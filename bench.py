@@ -1,0 +1,305 @@
+#!/usr/bin/env python
+"""bench.py — FP64 cell-updates/s of the ECHO RMHD step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 256] [--direction diag|x] [--impl reference]
+
+A "step" is one full SSP-RK3 time step (three passes of the whole hot path: INT+con2prim, three fused
+flux sweeps, UCT, curl+update) of the 3-D circularly-polarised Alfven wave on an n^3 periodic
+box, FP64; value = cells x steps / seconds, inputs resident in HBM.  Default workload: BASELINE.json
+configs[2] (256^3).  N > 1: every rank advances its own independent box (replicas, no collective; DESIGN.md
+"Multi-GPU"), value = sum over ranks / max time.  One JSON line on stdout (rank 0).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+GAMMA, CFL = 4.0 / 3.0, 0.3
+SETK = "rho vx vy vz p bxf byf bzf".split()
+
+# Algorithmic work per cell and per launch.
+# flop: nominal FP64 operation count of the scheme; dbl: FP64 words read+written once per cell.
+ALGO = {
+    "k_prim":   {"flop": 24 + 268, "dbl": 16},
+    "k_flux_x": {"flop": 614, "dbl": 17},
+    "k_flux_y": {"flop": 614, "dbl": 22},
+    "k_flux_z": {"flop": 614, "dbl": 22},
+    "k_uct":    {"flop": 3 * 194, "dbl": 18},
+    "k_update": {"flop": 60 + 32, "dbl": (24 + 32 + 32) / 3.0},
+}
+FLOP_PER_CELL_UPDATE = 3 * sum(v["flop"] for v in ALGO.values())          # 8424
+BYTES_PER_CELL_UPDATE = 8 * 3 * sum(v["dbl"] for v in ALGO.values())      # 2984
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    sm.append(float(f[1])); mx.append(float(f[2]))
+                except ValueError:
+                    continue
+                for nm, val in zip(names, f[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_rate(n, steps, warmup=0, direction="diag"):
+    """The oracle as it stands, single-threaded, on an n^3 box of the same wave: cell-updates/s."""
+    from oracle import binding as ob
+    from paper_2401_03008_b200 import inputs
+    w = inputs.cpa_wave(n, n, n, direction=direction)
+    o = ob.Oracle(n, n, n, GAMMA, CFL)
+    o.set_primitives(*[w[k] for k in SETK])
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return n ** 3 * steps / dt, dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, a bounded sample (48^3 box) per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = args.ref_n
+    rate, dt = oracle_rate(n, args.steps, args.warmup, args.direction)
+    sample = "%d^3 box of the same CPA wave (P:L217-233), %d RK3 steps, single thread" % (n, args.steps)
+    line = {"impl": "reference", "metric": "fp64_cell_updates_per_sec", "value": rate, "unit": "cell-updates/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "cpa_wave_%s_%d^3_oracle_sample" % (args.direction, n), "gamma": GAMMA, "cfl": CFL},
+            "cpu_baseline": {"value": rate, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_gpu(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2401_03008_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.lib()
+
+    n, K, W = args.n, args.steps, max(args.warmup, 3)
+    N = n ** 3
+    w = inputs.cpa_wave(n, n, n, direction=args.direction)
+    host = [torch.from_numpy(np.ascontiguousarray(w[k])).pin_memory() for k in SETK]
+    e = binding.Echo(n, n, n, GAMMA, CFL)
+    devin = [h.to("cuda", non_blocking=True) for h in host]
+    e.set_primitives(*devin)
+    del devin
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then EXACTLY K timed steps
+    e.step(W)
+    barrier()
+    e.timing(True)                      # per-kernel CUDA-event brackets on the launching stream
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    e.step(K)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    ktimes = e.get_timing()
+    e.timing(False)
+    d = e.diagnostics()
+    assert d["rc"] == 0 and d["steps"] == W + K, d
+    tt = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms_max = float(tt.item())
+    value = world * N * K / (ms_max * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: every step uploads its inputs from pinned host
+    # memory (echo_set_primitives_host), advances one RK3 step and reads the primitives back to the host
+    outs = [torch.empty(e.shape, dtype=torch.float64).pin_memory() for _ in range(8)]
+    Ke = min(K, args.e2e_steps)
+    for _ in range(2):
+        e.set_primitives_host(*host); e.step(1); e.get_primitives_host(outs)
+    barrier()
+    ev0.record()
+    for _ in range(Ke):
+        e.set_primitives_host(*host)
+        e.step(1)
+        e.get_primitives_host(outs)
+    ev1.record()
+    barrier()
+    te = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * N * Ke / (float(te.item()) * 1e-3)
+    # sanity of what came back: one step of the wave stays within truncation error of the input
+    assert abs(float(outs[0].mean()) - 1.0) < 1e-6
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (live CUDA-event durations of this run)
+    peaks, peak_kind = measured_peaks()
+    hbm_peak = float(peaks["hbm_gbs"])
+    fp64_burst, fp64_sust = binding.fp64_peak(20)
+    kernels = {}
+    for name, (tot, cnt) in ktimes.items():
+        if cnt and name in ALGO:
+            avg = tot / cnt
+            kernels[name] = {"ms_avg": avg, "launches": cnt, "share": tot / ms,
+                             "tflops": ALGO[name]["flop"] * N / (avg * 1e-3) * 1e-12,
+                             "gbs": 8 * ALGO[name]["dbl"] * N / (avg * 1e-3) * 1e-9}
+        elif cnt:
+            kernels[name] = {"ms_avg": tot / cnt, "launches": cnt, "share": tot / ms}
+    dom = max((k for k in kernels if k in ALGO), key=lambda k: kernels[k]["share"] * 1.0)
+    kd = kernels[dom]
+    t_alu = ALGO[dom]["flop"] / (fp64_sust * 1e12)
+    t_hbm = 8 * ALGO[dom]["dbl"] / (hbm_peak * 1e9)
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": kd["tflops"], "peak": fp64_sust, "unit": "TFLOP/s",
+                "frac": kd["tflops"] / fp64_sust}
+    else:
+        roof = {"bound": "hbm", "achieved": kd["gbs"], "peak": hbm_peak, "unit": "GB/s", "frac": kd["gbs"] / hbm_peak}
+    roof.update(kernel=dom, traffic=TRAFFIC.get(dom), peak_source=("FP64 DFMA micro-benchmark run by this bench "
+                "(sustained; burst %.1f)" % fp64_burst) if roof["bound"] == "alu" else "MEASURED_PEAKS.json (%s)" % peak_kind,
+                algorithmic_flop_per_cell=ALGO[dom]["flop"], algorithmic_bytes_per_cell=8 * ALGO[dom]["dbl"],
+                ms_per_launch=kd["ms_avg"], cells_per_launch=N)
+    step_bound = min(fp64_sust * 1e12 / FLOP_PER_CELL_UPDATE, hbm_peak * 1e9 / BYTES_PER_CELL_UPDATE)
+    per_gpu = value / world
+
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        rate, dt = oracle_rate(args.cpu_n, args.cpu_steps, 0, args.direction)
+        cpu = {"value": rate, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
+               "sample": "%d^3 box of the same CPA wave, %d RK3 steps, %.1f s, single thread" % (args.cpu_n, args.cpu_steps, dt)}
+
+    nlaunch = sum(cnt for _, cnt in ktimes.values())
+    line = {"metric": "fp64_cell_updates_per_sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "cpa_wave_%s_%d^3" % (args.direction, n), "grid": [n, n, n], "gamma": GAMMA, "cfl": CFL,
+                       "scheme": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)", "cells": N,
+                       "parallelism": "replicas x%d (no collective)" % world,
+                       "cache": "working set %.1f GB per GPU, far larger than the 126 MB L2" % (44 * 8 * N / 1e9)},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "cell-updates/s", "steps": Ke,
+                    "h2d_bytes_per_step": 8 * 8 * N, "d2h_bytes_per_step": 8 * 8 * N,
+                    "what": "per step: echo_set_primitives_host (8 fields, pinned) + echo_step(1) + echo_get_primitives_host (8 fields)"},
+            "gpu_launches": nlaunch,
+            "roofline": roof,
+            "step_roofline": {"bound_cell_updates_per_s": step_bound, "frac": per_gpu / step_bound,
+                              "flop_per_cell_update": FLOP_PER_CELL_UPDATE, "bytes_per_cell_update": BYTES_PER_CELL_UPDATE,
+                              "fp64_tflops_peak_measured": fp64_sust, "hbm_gbs_peak": hbm_peak,
+                              "achieved_tflops": per_gpu * FLOP_PER_CELL_UPDATE * 1e-12,
+                              "achieved_gbs": per_gpu * BYTES_PER_CELL_UPDATE * 1e-9},
+            "kernels": kernels,
+            "state": {"t": d["t"], "max_div_b": d["max_div_b"], "c2p_mean_iters": d["c2p_mean_iters"]},
+            "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+# (profiles/), keyed by kernel class; None until a capture of the current kernels exists.
+TRAFFIC = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
+    ap.add_argument("--n", type=int, default=256, help="box size n^3 (BASELINE.json configs[2]: 256)")
+    ap.add_argument("--direction", default="diag", choices=["diag", "x"])
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--cpu-n", type=int, default=64)
+    ap.add_argument("--cpu-steps", type=int, default=6)
+    ap.add_argument("--ref-n", type=int, default=48)
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

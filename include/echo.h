@@ -135,6 +135,28 @@ int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host);
  * 1e-15 is measurable.  Synchronises.  Returns ECHO_EC2P if the failure count is non-zero. */
 int echo_diagnostics(echo_ctx *ctx, double *out);
 
+/* ---- measurement aids (used by bench.py; not part of the numerical path) -------------------- */
+
+#define ECHO_NKCLASS 8
+/* Kernel classes of the per-kernel timers: 0 k_prim (INT+con2prim), 1..3 k_flux<x,y,z> (REC+HLL+DER+
+ * divergence), 4 k_uct, 5 k_update (curl+RK), 6 control kernels, 7 everything else. */
+
+/* enable != 0: from now on every kernel launch of this handle is bracketed by a CUDA-event pair on
+ * the bound stream (no synchronisation, no change to the launch order); also clears the timers and
+ * the launch counters.  enable == 0: stops bracketing. */
+int echo_timing(echo_ctx *ctx, int enable);
+
+/* Synchronises the stream; ms_total[c] (HOST, ECHO_NKCLASS doubles) = summed device time of class c
+ * since echo_timing(ctx, 1), launches[c] (HOST, ECHO_NKCLASS longs) = number of launches (counted
+ * whether or not timing is enabled, since the last echo_timing call or echo_bind). */
+int echo_get_timing(echo_ctx *ctx, double *ms_total, long *launches);
+
+/* FP64 vector-pipe peak of the current device, measured: `reps` launches of a register-resident
+ * kernel of independent DFMA chains (148 x 8 blocks x 256 threads), each timed with CUDA events on
+ * `cuda_stream`.  tflops_host[0] = best launch (burst), tflops_host[1] = all launches together
+ * (sustained).  Synchronises. */
+int echo_fp64_peak(int reps, double *tflops_host, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -35,7 +35,12 @@ SIGNATURES = {
     "echo_prim2cons": (_int, [_dbl, _long] + [_vp] * 13 + [_vp]),
     "echo_div_b": (_int, [_vp, _vp, C.POINTER(_dbl)]),
     "echo_diagnostics": (_int, [_vp, C.POINTER(_dbl)]),
+    "echo_timing": (_int, [_vp, _int]),
+    "echo_get_timing": (_int, [_vp, C.POINTER(_dbl), C.POINTER(_long)]),
+    "echo_fp64_peak": (_int, [_int, C.POINTER(_dbl), _vp]),
 }
+ECHO_NKCLASS = 8
+KCLASS_NAMES = ["k_prim", "k_flux_x", "k_flux_y", "k_flux_z", "k_uct", "k_update", "control", "other"]
 
 DIAG_NAMES = ["t", "dt_last", "steps", "amax", "sum_D", "sum_Sx", "sum_Sy", "sum_Sz", "sum_U",
               "sum_Bx", "sum_By", "sum_Bz", "max_div_b", "max_W", "min_rho", "min_p",
@@ -175,6 +180,28 @@ class Echo:
         d = dict(zip(DIAG_NAMES, list(out)[:len(DIAG_NAMES)]))
         d["rc"] = rc
         return d
+
+
+    # ---- measurement aids
+    def timing(self, enable=True):
+        self._check(self.L.echo_timing(self.h, 1 if enable else 0))
+
+    def get_timing(self):
+        """-> {class name: (total ms, launches)}; synchronises."""
+        ms = (_dbl * ECHO_NKCLASS)()
+        cnt = (_long * ECHO_NKCLASS)()
+        self._check(self.L.echo_get_timing(self.h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(KCLASS_NAMES)}
+
+
+def fp64_peak(reps=20):
+    """Measured FP64 DFMA peak of the current device in TFLOP/s: (burst, sustained)."""
+    _torch()
+    out = (_dbl * 2)()
+    rc = lib().echo_fp64_peak(int(reps), out, _stream())
+    if rc:
+        raise EchoError(rc, "echo_fp64_peak")
+    return out[0], out[1]
 
 
 def _host_ptr(a, n):

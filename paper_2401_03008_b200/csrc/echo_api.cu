@@ -24,6 +24,14 @@ struct echo_ctx {
     long long npad = 0;
     bool bound = false, has_state = false;
     std::string err;
+    // measurement aids (echo_timing / echo_get_timing)
+    bool timing = false;
+    long launches[ECHO_NKCLASS] = {0};
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    struct Span { int cls; size_t e0, e1; };
+    std::vector<Span> spans;
+    ~echo_ctx() { for (cudaEvent_t e : ev_pool) cudaEventDestroy(e); }
 };
 
 namespace {
@@ -48,6 +56,36 @@ int cuda_fail(echo_ctx *c, cudaError_t e, const char *where) {
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_, name);    \
     } while (0)
 
+// flux-sweep tiling: threads per block, transverse width, max tile length
+constexpr int FLUX_NT = 128, FLUX_TX = 4, FLUX_TYZ = 16, FLUX_LX = 64, FLUX_LYZ = 64;
+
+enum { KC_PRIM = 0, KC_FLUX = 1, KC_UCT = 4, KC_UPDATE = 5, KC_CTRL = 6, KC_OTHER = 7 };
+
+size_t next_event(echo_ctx *c) {
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        c->ev_pool.push_back(e);
+    }
+    cudaEventRecord(c->ev_pool[c->ev_used], c->stream);
+    return c->ev_used++;
+}
+void tbegin(echo_ctx *c, int cls) {
+    c->launches[cls]++;
+    if (c->timing) c->spans.push_back({cls, next_event(c), 0});
+}
+void tend(echo_ctx *c) {
+    if (c->timing) c->spans.back().e1 = next_event(c);
+}
+// launch of one kernel of class `cls`: counted, optionally bracketed by events, checked
+#define KL(cls, name, ...)        \
+    do {                          \
+        tbegin(ctx, cls);         \
+        __VA_ARGS__;              \
+        tend(ctx);                \
+        LAUNCH_CHECK(name);       \
+    } while (0)
+
 dim3 cell_block() { return dim3(64, 4, 1); }
 dim3 cell_grid(const Grid &g) { return dim3((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]); }
 
@@ -69,43 +107,36 @@ Stage make_stage(const echo_ctx *c, int which) {
 }
 
 template <int D>
-int launch_flux(echo_ctx *ctx, const Stage &st, const int *active, int want_amax) {
-    constexpr int NT = 128;
+int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax) {
+    constexpr int NT = FLUX_NT, T = (D == 0) ? FLUX_TX : FLUX_TYZ;
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
-    FluxTile tl;
-    const int Lmax = 64;
-    tl.T = (D == 0) ? 4 : 16;
-    tl.tilesD = (g.n[D] + Lmax - 1) / Lmax;
-    tl.L = (g.n[D] + tl.tilesD - 1) / tl.tilesD;
-    tl.tilesT = (g.n[TD] + tl.T - 1) / tl.T;
-    const size_t smem = sizeof(double) * 5 * (size_t)(tl.L + 5) * tl.T;
-    dim3 grid(tl.tilesT, tl.tilesD, g.n[OD]);
-    k_flux<D, NT><<<grid, NT, smem, ctx->stream>>>(g, st, tl, ctx->gamma, ctx->gg, ctx->ctrl, active, want_amax);
-    LAUNCH_CHECK("k_flux");
+    const int Lmax = (D == 0) ? FLUX_LX : FLUX_LYZ;
+    const int tilesD = (g.n[D] + Lmax - 1) / Lmax;
+    const int L = (g.n[D] + tilesD - 1) / tilesD;
+    const int tilesT = (g.n[TD] + T - 1) / T;
+    const size_t smem = sizeof(double) * 5 * (size_t)(L + 5) * T;
+    dim3 grid(tilesT, tilesD, g.n[OD]);
+    KL(KC_FLUX + D, "k_flux", k_flux<D, T, NT><<<grid, NT, smem, ctx->stream>>>(g, st, L, ctx->gamma, ctx->gg, ctx->ctrl, want_amax));
     return ECHO_OK;
 }
 
 // points 1-4 of a sub-step on the given stage pointers
-int launch_operator(echo_ctx *ctx, const Stage &st, const int *active, int want_amax) {
+int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax) {
     const Grid &g = ctx->g;
-    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, active);
-    LAUNCH_CHECK("k_prim");
+    KL(KC_PRIM, "k_prim", k_prim<false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
     int rc;
-    if ((rc = launch_flux<0>(ctx, st, active, want_amax))) return rc;
-    if ((rc = launch_flux<1>(ctx, st, active, want_amax))) return rc;
-    if ((rc = launch_flux<2>(ctx, st, active, want_amax))) return rc;
+    if ((rc = launch_flux<0>(ctx, st, want_amax))) return rc;
+    if ((rc = launch_flux<1>(ctx, st, want_amax))) return rc;
+    if ((rc = launch_flux<2>(ctx, st, want_amax))) return rc;
     if (want_amax == 2) {   // stage 1 of echo_step: dt must exist before the update (S9)
-        k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin);
-        LAUNCH_CHECK("k_set_dt");
+        KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
     }
-    k_uct<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, active);
-    LAUNCH_CHECK("k_uct");
+    KL(KC_UCT, "k_uct", k_uct<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st));
     return ECHO_OK;
 }
 
-int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, double c0, double c1,
-                  const int *active) {
+int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, double c0, double c1) {
     Update up;
     for (int v = 0; v < 8; ++v) {
         up.base[v] = ctx->field[F_U + v];
@@ -115,9 +146,8 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
     up.c0 = c0;
     up.c1 = c1;
     const Grid &g = ctx->g;
-    k_update<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1], st.R[2],
-                                                             st.R[3], st.R[4], up, ctx->ctrl, active);
-    LAUNCH_CHECK("k_update");
+    KL(KC_UPDATE, "k_update", k_update<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1], st.R[2],
+                                                             st.R[3], st.R[4], up, ctx->ctrl, 1));
     return ECHO_OK;
 }
 
@@ -135,12 +165,12 @@ extern "C" {
 echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl) {
     if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || !(cfl > 0.0) || !std::isfinite(gamma) || !std::isfinite(cfl))
         return nullptr;
-    if ((long long)nx * ny * nz > (1LL << 40) || nz > 65535 || ny > 4 * 65535) return nullptr;
+    if ((long long)nx * ny * nz >= (1LL << 31) - 64 || nz > 65535 || ny > 4 * 65535) return nullptr;   // 32-bit cell indices
     echo_ctx *c = new (std::nothrow) echo_ctx();
     if (!c) return nullptr;
     Grid &g = c->g;
     g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
-    g.s[0] = 1; g.s[1] = nx; g.s[2] = (long long)nx * ny;
+    g.s[0] = 1; g.s[1] = nx; g.s[2] = nx * ny;
     g.N = (long long)nx * ny * nz;
     for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; }
     c->gamma = gamma;
@@ -176,9 +206,9 @@ int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     h.one = 1;
     CU(cudaMemcpyAsync(ctx->ctrl, &h, sizeof(h), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));   // h is a stack object
-    CU(cudaFuncSetAttribute(k_flux<0, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-    CU(cudaFuncSetAttribute(k_flux<1, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-    CU(cudaFuncSetAttribute(k_flux<2, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CU(cudaFuncSetAttribute(k_flux<0, FLUX_TX, FLUX_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CU(cudaFuncSetAttribute(k_flux<1, FLUX_TYZ, FLUX_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+    CU(cudaFuncSetAttribute(k_flux<2, FLUX_TYZ, FLUX_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     ctx->bound = true;
     ctx->has_state = false;
     return ECHO_OK;
@@ -194,11 +224,10 @@ int echo_set_primitives(echo_ctx *ctx, const double *rho, const double *vx, cons
     for (int d = 0; d < 3; ++d)
         if (bf[d] != ctx->field[F_BF + d])
             CU(cudaMemcpyAsync(ctx->field[F_BF + d], bf[d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
-    k_init<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, rho, vx, vy, vz, p, ctx->field[F_BF], ctx->field[F_BF + 1],
+    KL(KC_OTHER, "k_init", k_init<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, rho, vx, vy, vz, p, ctx->field[F_BF], ctx->field[F_BF + 1],
                                                            ctx->field[F_BF + 2], ctx->field[F_U], ctx->field[F_U + 1],
                                                            ctx->field[F_U + 2], ctx->field[F_U + 3], ctx->field[F_U + 4],
-                                                           ctx->gg);
-    LAUNCH_CHECK("k_init");
+                                                           ctx->gg));
     Ctrl h;
     std::memset(&h, 0, sizeof(h));
     h.one = 1;
@@ -228,8 +257,7 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
     if (rc) return rc;
     if (!ax || !ay || !az || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
     const Grid &g = ctx->g;
-    k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ax, ay, az, bxf, byf, bzf, -1.0, b0x, b0y, b0z);
-    LAUNCH_CHECK("k_curl");
+    KL(KC_OTHER, "k_curl", k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ax, ay, az, bxf, byf, bzf, -1.0, b0x, b0y, b0z));
     return ECHO_OK;
 }
 
@@ -237,22 +265,19 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
-    const int *active = &ctx->ctrl->active;
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     for (int n = 0; n < nsteps; ++n) {
-        k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end);
-        LAUNCH_CHECK("k_begin_step");
+        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
         // stage 1: U1 = U^n + dt L(U^n), dt from the speeds of this very operator (S9)
-        if ((rc = launch_operator(ctx, s0, active, 2))) return rc;
-        if ((rc = launch_update(ctx, s0, 0, 1, 0.0, 1.0, active))) return rc;
+        if ((rc = launch_operator(ctx, s0, 2))) return rc;
+        if ((rc = launch_update(ctx, s0, 0, 1, 0.0, 1.0))) return rc;
         // stage 2: U2 = 3/4 U^n + 1/4 (U1 + dt L(U1))
-        if ((rc = launch_operator(ctx, s1, active, 0))) return rc;
-        if ((rc = launch_update(ctx, s1, 1, 1, 0.75, 0.25, active))) return rc;
+        if ((rc = launch_operator(ctx, s1, 0))) return rc;
+        if ((rc = launch_update(ctx, s1, 1, 1, 0.75, 0.25))) return rc;
         // stage 3: U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
-        if ((rc = launch_operator(ctx, s1, active, 0))) return rc;
-        if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, active))) return rc;
-        k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl);
-        LAUNCH_CHECK("k_end_step");
+        if ((rc = launch_operator(ctx, s1, 0))) return rc;
+        if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0))) return rc;
+        KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
     }
     return ECHO_OK;
 }
@@ -267,8 +292,7 @@ int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, doub
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 5; ++v) st.P[v] = out[v];
     for (int d = 0; d < 3; ++d) st.Bc[d] = out[5 + d];
-    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, &ctx->ctrl->one);
-    LAUNCH_CHECK("k_prim");
+    KL(KC_PRIM, "k_prim", k_prim<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
     double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d)
         if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -283,8 +307,7 @@ int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy,
     const Grid &g = ctx->g;
     const size_t nb = sizeof(double) * g.N;
     Stage st = make_stage(ctx, 0);
-    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, &ctx->ctrl->one);
-    LAUNCH_CHECK("k_prim");
+    KL(KC_PRIM, "k_prim", k_prim<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 8; ++v) CU(cudaMemcpyAsync(out[v], ctx->field[F_P + v], nb, cudaMemcpyDeviceToHost, ctx->stream));
     double *bf[3] = {bxf, byf, bzf};
@@ -312,15 +335,14 @@ int echo_rhs(echo_ctx *ctx, double *const *rhsU, double *const *rhsB, double *co
     const size_t nb = sizeof(double) * g.N;
     const Stage st = make_stage(ctx, 0);
     CU(cudaMemsetAsync(&ctx->ctrl->amax_bits, 0, sizeof(unsigned long long), ctx->stream));
-    if ((rc = launch_operator(ctx, st, &ctx->ctrl->one, 1))) return rc;
+    if ((rc = launch_operator(ctx, st, 1))) return rc;
     if (rhsU)
         for (int v = 0; v < 5; ++v) CU(cudaMemcpyAsync(rhsU[v], st.R[v], nb, cudaMemcpyDeviceToDevice, ctx->stream));
     if (E)
         for (int d = 0; d < 3; ++d) CU(cudaMemcpyAsync(E[d], st.E[d], nb, cudaMemcpyDeviceToDevice, ctx->stream));
     if (rhsB) {
-        k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], rhsB[0], rhsB[1], rhsB[2],
-                                                               1.0, 0.0, 0.0, 0.0);
-        LAUNCH_CHECK("k_curl");
+        KL(KC_OTHER, "k_curl", k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], rhsB[0], rhsB[1], rhsB[2],
+                                                               1.0, 0.0, 0.0, 0.0));
     }
     if (amax_host) {
         unsigned long long bits = 0;
@@ -361,9 +383,8 @@ int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host) {
     const Grid &g = ctx->g;
     double *slot = ctx->part + 15 * NPART;   // spare partial row: one double for the max
     CU(cudaMemsetAsync(slot, 0, sizeof(double), ctx->stream));
-    k_divb<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ctx->field[F_BF], ctx->field[F_BF + 1], ctx->field[F_BF + 2],
-                                                           div_field, slot);
-    LAUNCH_CHECK("k_divb");
+    KL(KC_OTHER, "k_divb", k_divb<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ctx->field[F_BF], ctx->field[F_BF + 1],
+                                                                                  ctx->field[F_BF + 2], div_field, slot));
     double m = 0.0;
     CU(cudaMemcpyAsync(&m, slot, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -379,15 +400,12 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
     for (int m = 0; m < ECHO_NDIAG; ++m) out[m] = 0.0;
     double *f = ctx->field[F_U];
     const long long np = ctx->npad;
-    k_sums<<<NPART, 256, 0, ctx->stream>>>(g.N, f, f + np, f + 2 * np, f + 3 * np, f + 4 * np, f + 5 * np, f + 6 * np,
-                                           f + 7 * np, ctx->part);
-    LAUNCH_CHECK("k_sums");
+    KL(KC_OTHER, "k_sums", k_sums<<<NPART, 256, 0, ctx->stream>>>(g.N, f, f + np, f + 2 * np, f + 3 * np, f + 4 * np, f + 5 * np, f + 6 * np,
+                                           f + 7 * np, ctx->part));
     Stage st = make_stage(ctx, 0);
-    k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl);
-    k_prim<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, &ctx->ctrl->one);
-    LAUNCH_CHECK("k_prim");
-    k_extrema<<<NPART, 256, 0, ctx->stream>>>(g.N, st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], ctx->part);
-    LAUNCH_CHECK("k_extrema");
+    KL(KC_CTRL, "k_c2p_stats_reset", k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+    KL(KC_PRIM, "k_prim", k_prim<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
+    KL(KC_OTHER, "k_extrema", k_extrema<<<NPART, 256, 0, ctx->stream>>>(g.N, st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], ctx->part));
     double dmax = 0.0;
     if ((rc = echo_div_b(ctx, nullptr, &dmax))) return rc;   // synchronises
     std::vector<double> part((size_t)NPART * 11);
@@ -416,6 +434,64 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
     out[17] = h.c2p_calls ? (double)h.c2p_sumit / (double)h.c2p_calls : 0.0;
     out[18] = (double)h.c2p_fail_total;
     return h.c2p_fail_total ? fail(ctx, ECHO_EC2P, "con2prim failed in at least one cell") : ECHO_OK;
+}
+
+int echo_timing(echo_ctx *ctx, int enable) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->timing = enable != 0;
+    ctx->spans.clear();
+    ctx->ev_used = 0;
+    for (int c = 0; c < ECHO_NKCLASS; ++c) ctx->launches[c] = 0;
+    return ECHO_OK;
+}
+
+int echo_get_timing(echo_ctx *ctx, double *ms_total, long *launches) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (ms_total) {
+        for (int c = 0; c < ECHO_NKCLASS; ++c) ms_total[c] = 0.0;
+        for (const echo_ctx::Span &s : ctx->spans) {
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, ctx->ev_pool[s.e0], ctx->ev_pool[s.e1]));
+            ms_total[s.cls] += ms;
+        }
+    }
+    if (launches)
+        for (int c = 0; c < ECHO_NKCLASS; ++c) launches[c] = ctx->launches[c];
+    return ECHO_OK;
+}
+
+int echo_fp64_peak(int reps, double *tflops_host, void *cuda_stream) {
+    if (reps < 1 || !tflops_host) return ECHO_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int blocks = 148 * 8, threads = 256, iters = 4096;
+    double *sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return ECHO_ECUDA;
+    std::vector<cudaEvent_t> ev(reps + 1);
+    for (auto &e : ev) cudaEventCreate(&e);
+    k_dfma_peak<<<blocks, threads, 0, st>>>(iters, 1.0000001, sink);   // warm-up
+    cudaEventRecord(ev[0], st);
+    for (int r = 0; r < reps; ++r) {
+        k_dfma_peak<<<blocks, threads, 0, st>>>(iters, 1.0000001, sink);
+        cudaEventRecord(ev[r + 1], st);
+    }
+    cudaError_t e = cudaStreamSynchronize(st);
+    const double flop = 2.0 * DFMA_CHAINS * (double)iters * blocks * threads;
+    double best = 0.0;
+    float ms = 0.f;
+    for (int r = 0; r < reps && e == cudaSuccess; ++r) {
+        cudaEventElapsedTime(&ms, ev[r], ev[r + 1]);
+        best = std::fmax(best, flop / (ms * 1e-3) * 1e-12);
+    }
+    cudaEventElapsedTime(&ms, ev[0], ev[reps]);
+    tflops_host[0] = best;
+    tflops_host[1] = flop * reps / (ms * 1e-3) * 1e-12;
+    for (auto &x : ev) cudaEventDestroy(x);
+    cudaFree(sink);
+    return e == cudaSuccess ? ECHO_OK : ECHO_ECUDA;
 }
 
 }  // extern "C"

@@ -51,8 +51,12 @@ __global__ void k_c2p_stats_reset(Ctrl *c) {
 
 // ------------------------------------------------------------------ point 1: INT + con2prim
 // One thread per cell, block (64,4,1).  Face B comes in through L1/L2 with 6-point stencils.
-__global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, const int *active) {
-    if (!*active) return;
+// STATS: iteration statistics for echo_diagnostics (block reduction, one atomic set per block);
+// inside echo_step only failures are counted (no atomics at all on healthy data).
+// Divergent Newton counts: each lane runs its own loop and freezes at its own convergence, so a
+// cell's result never depends on which cells share its warp (translation covariance stays bitwise).
+template <bool STATS>
+__global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
@@ -60,41 +64,44 @@ __global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl
     const bool in = (i < g.n[0]) && (j < g.n[1]);
     if (in) {
         const int c3[3] = {i, j, k};
-        const long long c = i + g.s[1] * j + g.s[2] * k;
+        const int c = i + g.s[1] * j + g.s[2] * k;
         double B[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            const long long base = c - g.s[d] * c3[d];
+            const int base = c - g.s[d] * c3[d];
             double b[6];
 #pragma unroll
-            for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]));
+            for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
             B[d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
         }
-        const double u[5] = {st.U[0][c], st.U[1][c], st.U[2][c], st.U[3][c], st.U[4][c]};
+        const double u[5] = {__ldg(st.U[0] + c), __ldg(st.U[1] + c), __ldg(st.U[2] + c), __ldg(st.U[3] + c),
+                             __ldg(st.U[4] + c)};
         double q[5];
         it = con2prim(gam, u, B, q);
 #pragma unroll
         for (int v = 0; v < 5; ++v) st.P[v][c] = q[v];
 #pragma unroll
         for (int d = 0; d < 3; ++d) st.Bc[d][c] = B[d];
+        if (it < 0) atomicAdd(&ctrl->c2p_fail_total, 1ull);
     }
-    // statistics: warp reduction, one atomic per warp
-    const int ai = it < 0 ? -it : it;
-    int sum = ai, mx = ai, fail = it < 0 ? 1 : 0, calls = in ? 1 : 0;
+    if (STATS) {
+        __shared__ int s_sum[8], s_max[8], s_cnt[8];
+        const int ai = it < 0 ? -it : it;
+        int sum = ai, mx = ai, calls = in ? 1 : 0;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        sum += __shfl_xor_sync(0xffffffffu, sum, o);
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        fail += __shfl_xor_sync(0xffffffffu, fail, o);
-        calls += __shfl_xor_sync(0xffffffffu, calls, o);
-    }
-    if (((threadIdx.y * blockDim.x + threadIdx.x) & 31) == 0) {
-        atomicAdd(&ctrl->c2p_sumit, (unsigned long long)sum);
-        atomicAdd(&ctrl->c2p_calls, (unsigned long long)calls);
-        atomicMax(&ctrl->c2p_maxit, mx);
-        if (fail) {
-            atomicAdd(&ctrl->c2p_fail, (unsigned long long)fail);
-            atomicAdd(&ctrl->c2p_fail_total, (unsigned long long)fail);
+        for (int o = 16; o > 0; o >>= 1) {
+            sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            calls += __shfl_xor_sync(0xffffffffu, calls, o);
+        }
+        const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+        if ((tid & 31) == 0) { s_sum[tid >> 5] = sum; s_max[tid >> 5] = mx; s_cnt[tid >> 5] = calls; }
+        __syncthreads();
+        if (tid == 0) {
+            for (int w = 1; w < 8; ++w) { sum += s_sum[w]; mx = max(mx, s_max[w]); calls += s_cnt[w]; }
+            atomicAdd(&ctrl->c2p_sumit, (unsigned long long)sum);
+            atomicAdd(&ctrl->c2p_calls, (unsigned long long)calls);
+            atomicMax(&ctrl->c2p_maxit, mx);
         }
     }
 }
@@ -109,15 +116,15 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
     const int k = blockIdx.z;
     if (i >= g.n[0] || j >= g.n[1]) return;
     const int c3[3] = {i, j, k};
-    const long long c = i + g.s[1] * j + g.s[2] * k;
+    const int c = i + g.s[1] * j + g.s[2] * k;
     const double *bf[3] = {bf0, bf1, bf2};
     double q[8] = {rho[c], vx[c], vy[c], vz[c], p[c], 0.0, 0.0, 0.0};
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        const long long base = c - g.s[d] * c3[d];
+        const int base = c - g.s[d] * c3[d];
         double b[6];
 #pragma unroll
-        for (int m = 0; m < 6; ++m) b[m] = __ldg(bf[d] + base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]));
+        for (int m = 0; m < 6; ++m) b[m] = __ldg(bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
         q[5 + d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
     }
     double u[5];
@@ -133,95 +140,121 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
 // Phase 2: rhs -= (F^_{i+1/2} - F^_{i-1/2})/h_D from shared memory (DER).  The 5 halo
 // faces are recomputed by the neighbouring tile with the same instructions on the same inputs,
 // hence bit-identically: conservation stays at round-off.
-struct FluxTile { int L, T, tilesD, tilesT; };
-
-template <int D, int NT>
-__global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, FluxTile tl, double gam, double gg, Ctrl *ctrl,
-                                             const int *active, int want_amax) {
-    if (!*active) return;
+// REC: all 14 unlimited MP5 values and their S&H tests first; the limiter itself runs out of line
+// only for the (field, side) pairs whose test fired (never on smooth data).
+template <int D, int T, int NT>
+__global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int L, double gam, double gg, Ctrl *ctrl,
+                                             int want_amax) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
     constexpr int OD = 3 - D - TD;            // remaining axis
     constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
     extern __shared__ double sF[];
-    const int L = tl.L, T = tl.T, LA = L + 5;
-    const int tileT = blockIdx.x, tileD = blockIdx.y;
-    const int cO = blockIdx.z;
-    const int m0 = tileD * L;
-    const int t0 = tileT * T;
+    const int LA = L + 5;
+    const int m0 = blockIdx.y * L;
+    const int t0 = blockIdx.x * T;
     const int nD = g.n[D], nT = g.n[TD];
     const int Lv = min(L, nD - m0);           // valid cells of this tile along D
-    const long long sD = g.s[D], sT = g.s[TD];
-    const long long baseO = g.s[OD] * cO;
+    const int sD = g.s[D], sT = g.s[TD];
+    const int baseO = g.s[OD] * (int)blockIdx.z;
     const int nface = LA * T;
     double amax = 0.0;
 
+    // face slot f -> (a along D, b along TD); lanes run along the contiguous axis
+    int a, b;
+    if (D == 0) { a = threadIdx.x % LA; b = threadIdx.x / LA; } else { b = threadIdx.x % T; a = threadIdx.x / T; }
     for (int f = threadIdx.x; f < nface; f += NT) {
-        int a, b;
-        if (D == 0) { a = f % LA; b = f / LA; } else { b = f % T; a = f / T; }
         const int cT = t0 + b;
-        if (cT >= nT || a >= Lv + 5) continue;
-        const int m = m0 - 3 + a;             // face m sits between cells m and m+1
-        long long idx[6];
+        if (cT < nT && a < Lv + 5) {
+            const int m = m0 - 3 + a;             // face m sits between cells m and m+1
+            const int base = baseO + sT * cT;
+            int idx[6];
 #pragma unroll
-        for (int s = 0; s < 6; ++s) idx[s] = baseO + sT * cT + sD * wrapi(m - 2 + s, nD);
-        double qL[8], qR[8];
-        {
-            const double *rec[7] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2]};
-            const int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+            for (int s = 0; s < 6; ++s) idx[s] = base + sD * wrapi(m - 2 + s, nD);
+            double qL[8], qR[8];
+            unsigned need = 0u;
+            {
+                const double *rec[7] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2]};
+                const int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
 #pragma unroll
-            for (int v = 0; v < 7; ++v) {
-                double s[6];
+                for (int v = 0; v < 7; ++v) {
+                    double s[6];
 #pragma unroll
-                for (int k = 0; k < 6; ++k) s[k] = __ldg(rec[v] + idx[k]);
-                qL[slot[v]] = mp5(s[0], s[1], s[2], s[3], s[4]);
-                qR[slot[v]] = mp5(s[5], s[4], s[3], s[2], s[1]);
+                    for (int k = 0; k < 6; ++k) s[k] = __ldg(rec[v] + idx[k]);
+                    bool nl, nr;
+                    qL[slot[v]] = mp5_fast(s[0], s[1], s[2], s[3], s[4], nl);
+                    qR[slot[v]] = mp5_fast(s[5], s[4], s[3], s[2], s[1], nr);
+                    need |= (nl ? 1u : 0u) << (2 * v) | (nr ? 1u : 0u) << (2 * v + 1);
+                }
+                if (need) {
+#pragma unroll 1
+                    for (int v = 0; v < 7; ++v) {
+                        const unsigned bits = (need >> (2 * v)) & 3u;
+                        if (!bits) continue;
+                        const double *fp = rec[0];
+#pragma unroll
+                        for (int w = 1; w < 7; ++w) fp = (v == w) ? rec[w] : fp;
+                        double s[6];
+#pragma unroll
+                        for (int k = 0; k < 6; ++k) s[k] = __ldg(fp + idx[k]);
+                        const double lim_l = (bits & 1u) ? mp5_limited(s[0], s[1], s[2], s[3], s[4]) : 0.0;
+                        const double lim_r = (bits & 2u) ? mp5_limited(s[5], s[4], s[3], s[2], s[1]) : 0.0;
+#pragma unroll
+                        for (int w = 0; w < 7; ++w) {
+                            if (w == v && (bits & 1u)) qL[slot[w]] = lim_l;
+                            if (w == v && (bits & 2u)) qR[slot[w]] = lim_r;
+                        }
+                    }
+                }
+            }
+            qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + idx[2]);   // the normal B is the staggered value
+            double F[5], ap, am, vb1, vb2;
+            hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
+            const int so = (D == 0) ? (b * LA + a) : (a * T + b);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) sF[c * nface + so] = F[c];
+            if (a >= 3 && a < Lv + 3) {
+                const int o = idx[2];
+                st.ap[D][o] = ap;
+                st.am[D][o] = am;
+                st.vb[D][0][o] = vb1;
+                st.vb[D][1][o] = vb2;
+                amax = dmax(amax, dmax(ap, am));
             }
         }
-        qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + idx[2]);   // the normal B is the staggered value
-        double F[5], ap, am, vb1, vb2;
-        hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
-        const int so = (D == 0) ? (b * LA + a) : (a * T + b);
-#pragma unroll
-        for (int c = 0; c < 5; ++c) sF[c * nface + so] = F[c];
-        if (a >= 3 && a < Lv + 3) {
-            const long long o = idx[2];
-            st.ap[D][o] = ap;
-            st.am[D][o] = am;
-            st.vb[D][0][o] = vb1;
-            st.vb[D][1][o] = vb2;
-            amax = fmax(amax, fmax(ap, am));
-        }
+        if (D == 0) { a += NT; while (a >= LA) { a -= LA; ++b; } } else { a += NT / T; }
     }
     __syncthreads();
 
-    const double rh = g.rh[D];
+    const double mrh = -g.rh[D];
     const int ncell = L * T;
+    if (D == 0) { a = threadIdx.x % L; b = threadIdx.x / L; } else { b = threadIdx.x % T; a = threadIdx.x / T; }
     for (int e = threadIdx.x; e < ncell; e += NT) {
-        int a, b;
-        if (D == 0) { a = e % L; b = e / L; } else { b = e % T; a = e / T; }
         const int cT = t0 + b;
-        if (cT >= nT || a >= Lv) continue;
-        const long long o = baseO + sT * cT + sD * (m0 + a);
-        const int step = (D == 0) ? 1 : T;
-        const int so = (D == 0) ? (b * LA + a) : (a * T + b);
+        if (cT < nT && a < Lv) {
+            const int o = baseO + sT * cT + sD * (m0 + a);
+            constexpr int one = 1;
+            const int step = (D == 0) ? one : T;
+            const int so = (D == 0) ? (b * LA + a) : (a * T + b);
 #pragma unroll
-        for (int c = 0; c < 5; ++c) {
-            const double *F = sF + c * nface + so;
-            const double r = -rh * der_diff(F[0], F[step], F[2 * step], F[3 * step], F[4 * step], F[5 * step]);
-            if (D == 0) st.R[c][o] = r; else st.R[c][o] += r;
+            for (int c = 0; c < 5; ++c) {
+                const double *F = sF + c * nface + so;
+                const double r = mrh * der_diff(F[0], F[step], F[2 * step], F[3 * step], F[4 * step], F[5 * step]);
+                if (D == 0) st.R[c][o] = r; else st.R[c][o] += r;
+            }
         }
+        if (D == 0) { a += NT; while (a >= L) { a -= L; ++b; } } else { a += NT / T; }
     }
 
     if (want_amax) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        for (int o = 16; o > 0; o >>= 1) amax = dmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
         __shared__ double wmax[NT / 32];
         if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = amax;
         __syncthreads();
         if (threadIdx.x == 0) {
             double m = wmax[0];
 #pragma unroll
-            for (int w = 1; w < NT / 32; ++w) m = fmax(m, wmax[w]);
+            for (int w = 1; w < NT / 32; ++w) m = dmax(m, wmax[w]);
             atomic_max_nonneg(&ctrl->amax_bits, m);
         }
     }
@@ -233,46 +266,66 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, FluxTile tl, doub
 // where (vbar_i saved at j-faces, staggered B_j) are MP5-reconstructed along i and the edge speeds
 // are the max of the saved face speeds over the two faces adjacent to the edge.
 template <int K>
-__device__ __forceinline__ double uct_edge(const Stage &st, const long long (*ix)[6], long long c) {
+__device__ __forceinline__ double uct_edge(const Stage &st, const int (*ix)[6], int c) {
     constexpr int I = (K + 1) % 3, J = (K + 2) % 3;
     // slots: direction J saves vbar_{(J+1)%3} = vbar_K in [0], vbar_{(J+2)%3} = vbar_I in [1];
     //        direction I saves vbar_{(I+1)%3} = vbar_J in [0]
-    const double *vi = st.vb[J][1], *vj = st.vb[I][0];
-    const double *Bi = st.Bf[I], *Bj = st.Bf[J];
-    double s[6];
+    // q = 0: vbar_i along i, 1: B_j along i, 2: vbar_j along j, 3: B_i along j
+    const double *fld[4] = {st.vb[J][1], st.Bf[J], st.vb[I][0], st.Bf[I]};
+    double L[4], R[4];
+    unsigned need = 0u;
 #pragma unroll
-    for (int m = 0; m < 6; ++m) s[m] = __ldg(vi + ix[I][m]);
-    const double viL = mp5(s[0], s[1], s[2], s[3], s[4]), viR = mp5(s[5], s[4], s[3], s[2], s[1]);
+    for (int q = 0; q < 4; ++q) {
+        const int *x = ix[q < 2 ? I : J];
+        double s[6];
 #pragma unroll
-    for (int m = 0; m < 6; ++m) s[m] = __ldg(Bj + ix[I][m]);
-    const double BjL = mp5(s[0], s[1], s[2], s[3], s[4]), BjR = mp5(s[5], s[4], s[3], s[2], s[1]);
+        for (int m = 0; m < 6; ++m) s[m] = __ldg(fld[q] + x[m]);
+        bool nl, nr;
+        L[q] = mp5_fast(s[0], s[1], s[2], s[3], s[4], nl);
+        R[q] = mp5_fast(s[5], s[4], s[3], s[2], s[1], nr);
+        need |= (nl ? 1u : 0u) << (2 * q) | (nr ? 1u : 0u) << (2 * q + 1);
+    }
+    if (need) {
+#pragma unroll 1
+        for (int q = 0; q < 4; ++q) {
+            const unsigned bits = (need >> (2 * q)) & 3u;
+            if (!bits) continue;
+            const double *fp = fld[0];
 #pragma unroll
-    for (int m = 0; m < 6; ++m) s[m] = __ldg(vj + ix[J][m]);
-    const double vjL = mp5(s[0], s[1], s[2], s[3], s[4]), vjR = mp5(s[5], s[4], s[3], s[2], s[1]);
+            for (int w = 1; w < 4; ++w) fp = (q == w) ? fld[w] : fp;
+            double s[6];
 #pragma unroll
-    for (int m = 0; m < 6; ++m) s[m] = __ldg(Bi + ix[J][m]);
-    const double BiL = mp5(s[0], s[1], s[2], s[3], s[4]), BiR = mp5(s[5], s[4], s[3], s[2], s[1]);
-    const long long cj = ix[J][3], ci = ix[I][3];   // neighbours +1 along j and along i
-    const double aip = fmax(__ldg(st.ap[I] + c), __ldg(st.ap[I] + cj));
-    const double aim = fmax(__ldg(st.am[I] + c), __ldg(st.am[I] + cj));
-    const double ajp = fmax(__ldg(st.ap[J] + c), __ldg(st.ap[J] + ci));
-    const double ajm = fmax(__ldg(st.am[J] + c), __ldg(st.am[J] + ci));
-    return -(aip * viL * BjL + aim * viR * BjR - aip * aim * (BjR - BjL)) / (aip + aim) +
-           (ajp * vjL * BiL + ajm * vjR * BiR - ajp * ajm * (BiR - BiL)) / (ajp + ajm);
+            for (int m = 0; m < 6; ++m) s[m] = __ldg(fp + (q < 2 ? ix[I][m] : ix[J][m]));
+            const double lim_l = (bits & 1u) ? mp5_limited(s[0], s[1], s[2], s[3], s[4]) : 0.0;
+            const double lim_r = (bits & 2u) ? mp5_limited(s[5], s[4], s[3], s[2], s[1]) : 0.0;
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                if (w == q && (bits & 1u)) L[w] = lim_l;
+                if (w == q && (bits & 2u)) R[w] = lim_r;
+            }
+        }
+    }
+    const int cj = ix[J][3], ci = ix[I][3];   // neighbours +1 along j and along i
+    const double aip = dmax(__ldg(st.ap[I] + c), __ldg(st.ap[I] + cj));
+    const double aim = dmax(__ldg(st.am[I] + c), __ldg(st.am[I] + cj));
+    const double ajp = dmax(__ldg(st.ap[J] + c), __ldg(st.ap[J] + ci));
+    const double ajm = dmax(__ldg(st.am[J] + c), __ldg(st.am[J] + ci));
+    const double viL = L[0], viR = R[0], BjL = L[1], BjR = R[1], vjL = L[2], vjR = R[2], BiL = L[3], BiR = R[3];
+    return -(aip * viL * BjL + aim * viR * BjR - aip * aim * (BjR - BjL)) * rcp_fast(aip + aim) +
+           (ajp * vjL * BiL + ajm * vjR * BiR - ajp * ajm * (BiR - BiL)) * rcp_fast(ajp + ajm);
 }
 
-__global__ void __launch_bounds__(256) k_uct(Grid g, Stage st, const int *active) {
-    if (!*active) return;
+__global__ void __launch_bounds__(256) k_uct(Grid g, Stage st) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
     if (i >= g.n[0] || j >= g.n[1]) return;
     const int c3[3] = {i, j, k};
-    const long long c = i + g.s[1] * j + g.s[2] * k;
-    long long ix[3][6];   // cells c-2 .. c+3 along each axis
+    const int c = i + g.s[1] * j + g.s[2] * k;
+    int ix[3][6];   // cells c-2 .. c+3 along each axis
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        const long long base = c - g.s[d] * c3[d];
+        const int base = c - g.s[d] * c3[d];
 #pragma unroll
         for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 2, g.n[d]);
     }
@@ -284,9 +337,11 @@ __global__ void __launch_bounds__(256) k_uct(Grid g, Stage st, const int *active
 // ------------------------------------------------------------------ points 4b + 5: curl + RK update
 // rhs of the staggered B (O8, eq.(10)): dB_i/dt = -[ D_j(DER_j E_k) - D_k(DER_k E_j) ],
 // then for all 8 evolved fields  out = c0*base + c1*(cur + dt*rhs)  (O9).
-// dt is read from the device control block (a8: no host round trip).
+// dt is read from the device control block (a8: no host round trip).  This is the only kernel that
+// honours ctrl->active: once t >= t_end a step must leave the state untouched, and only the update
+// writes state (every other kernel writes scratch).
 template <int I>
-__device__ __forceinline__ double curl_comp(const Grid &g, const double *const E[3], const long long (*ix)[6]) {
+__device__ __forceinline__ double curl_comp(const Grid &g, const double *const E[3], const int (*ix)[6]) {
     constexpr int J = (I + 1) % 3, K = (I + 2) % 3;
     double a[6], b[6];
 #pragma unroll
@@ -298,27 +353,28 @@ __device__ __forceinline__ double curl_comp(const Grid &g, const double *const E
 __global__ void __launch_bounds__(256) k_update(Grid g, const double *E0, const double *E1, const double *E2,
                                                 const double *R0, const double *R1, const double *R2,
                                                 const double *R3, const double *R4, Update up, const Ctrl *ctrl,
-                                                const int *active) {
-    if (!*active) return;
+                                                int honour_active) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
     if (i >= g.n[0] || j >= g.n[1]) return;
-    const int c3[3] = {i, j, k};
-    const long long c = i + g.s[1] * j + g.s[2] * k;
     const double dt = ctrl->dt;
-    long long ix[3][6];   // cells c-3 .. c+2 along each axis (faces/edges i-5/2 .. i+5/2 of the difference)
+    const int active = ctrl->active;
+    const int c3[3] = {i, j, k};
+    const int c = i + g.s[1] * j + g.s[2] * k;
+    int ix[3][6];   // cells c-3 .. c+2 along each axis (faces/edges i-5/2 .. i+5/2 of the difference)
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        const long long base = c - g.s[d] * c3[d];
+        const int base = c - g.s[d] * c3[d];
 #pragma unroll
         for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]);
     }
     const double *const E[3] = {E0, E1, E2};
-    double r[8] = {R0[c], R1[c], R2[c], R3[c], R4[c], 0.0, 0.0, 0.0};
+    double r[8] = {__ldg(R0 + c), __ldg(R1 + c), __ldg(R2 + c), __ldg(R3 + c), __ldg(R4 + c), 0.0, 0.0, 0.0};
     r[5] = curl_comp<0>(g, E, ix);
     r[6] = curl_comp<1>(g, E, ix);
     r[7] = curl_comp<2>(g, E, ix);
+    if (honour_active && !active) return;
 #pragma unroll
     for (int v = 0; v < 8; ++v) {
         const double cur = up.cur[v][c];
@@ -327,7 +383,7 @@ __global__ void __launch_bounds__(256) k_update(Grid g, const double *E0, const 
     }
 }
 
-// rhs of B alone (echo_rhs) and B = curl A (echo_faces_from_potential, sign = +1, S11)
+// rhs of B alone (echo_rhs) and B = curl A (echo_faces_from_potential, sign = -1, S11)
 __global__ void __launch_bounds__(256) k_curl(Grid g, const double *E0, const double *E1, const double *E2,
                                               double *o0, double *o1, double *o2, double sign, double b0x,
                                               double b0y, double b0z) {
@@ -336,11 +392,11 @@ __global__ void __launch_bounds__(256) k_curl(Grid g, const double *E0, const do
     const int k = blockIdx.z;
     if (i >= g.n[0] || j >= g.n[1]) return;
     const int c3[3] = {i, j, k};
-    const long long c = i + g.s[1] * j + g.s[2] * k;
-    long long ix[3][6];
+    const int c = i + g.s[1] * j + g.s[2] * k;
+    int ix[3][6];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        const long long base = c - g.s[d] * c3[d];
+        const int base = c - g.s[d] * c3[d];
 #pragma unroll
         for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]);
     }
@@ -360,14 +416,14 @@ __global__ void __launch_bounds__(256) k_divb(Grid g, const double *B0, const do
     double v = 0.0;
     if (i < g.n[0] && j < g.n[1]) {
         const int c3[3] = {i, j, k};
-        const long long c = i + g.s[1] * j + g.s[2] * k;
+        const int c = i + g.s[1] * j + g.s[2] * k;
         const double *B[3] = {B0, B1, B2};
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            const long long base = c - g.s[d] * c3[d];
+            const int base = c - g.s[d] * c3[d];
             double f[6];
 #pragma unroll
-            for (int m = 0; m < 6; ++m) f[m] = __ldg(B[d] + base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]));
+            for (int m = 0; m < 6; ++m) f[m] = __ldg(B[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
             v += g.rh[d] * der_diff(f[0], f[1], f[2], f[3], f[4], f[5]);
         }
         if (div) div[c] = v;
@@ -465,4 +521,24 @@ __global__ void __launch_bounds__(256) k_p2c_batch(double gg, long long n, const
     }
 }
 
+}  // namespace echo
+
+// ------------------------------------------------------------------ FP64 peak micro-benchmark
+// Register-resident independent DFMA chains: the denominator of the ALU roofline.
+namespace echo {
+constexpr int DFMA_CHAINS = 8;
+__global__ void __launch_bounds__(256) k_dfma_peak(int iters, double a, double *sink) {
+    double x[DFMA_CHAINS];
+#pragma unroll
+    for (int c = 0; c < DFMA_CHAINS; ++c) x[c] = 1.0 + 1e-3 * (threadIdx.x + c);
+    const double b = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int c = 0; c < DFMA_CHAINS; ++c) x[c] = fma(x[c], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < DFMA_CHAINS; ++c) s += x[c];
+    if (s == 12345.678) *sink = s;   // never true: keeps the chains alive
+}
 }  // namespace echo

@@ -23,23 +23,64 @@ __device__ __forceinline__ double der_diff(double f0, double f1, double f2, doub
     return (75.0 / 64.0) * (f3 - f2) + ((-25.0 / 384.0) * (f4 - f1) + (3.0 / 640.0) * (f5 - f0));
 }
 
+// ---------------------------------------------------------------- fast FP64 helpers
+// min / max without the IEEE NaN bookkeeping of fmin/fmax (one DSETP + selects)
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+
+// Reciprocal, reciprocal square root and square root for NORMAL positive arguments: the MUFU
+// seed (about 20 good bits) refined by one third-order step (error ~ e^3, then rounding), ~1 ulp.
+// No denormal / special-case slow path: the arguments here are O(1) physical quantities; a zero
+// or negative argument yields inf/NaN exactly like the exact operation would, and propagates.
+__device__ __forceinline__ double rcp_fast(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y * e, 1.0 + e, y);
+}
+__device__ __forceinline__ double rsqrt_fast(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
+}
+__device__ __forceinline__ double sqrt_fast(double x) {   // x >= 0; exact 0 -> 0
+    const double y = rsqrt_fast(x);
+    const double s = x * y;
+    const double r = fma(-s, s, x);
+    const double t = fma(r, 0.5 * y, s);
+    return x > 0.0 ? t : 0.0;
+}
+
 __device__ __forceinline__ double minmod2(double a, double b) {
-    // same sign: the one of smaller magnitude; else 0
-    const double m = fmin(fabs(a), fabs(b));
-    return (a * b > 0.0) ? copysign(m, a) : 0.0;
+    // same sign: the one of smaller magnitude; else 0.  The sign test is done on the high words
+    // (integer pipe); a zero argument selects itself as the smaller magnitude, so it needs no test.
+    const double m = (fabs(a) < fabs(b)) ? a : b;
+    return ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
 }
 __device__ __forceinline__ double minmod4(double a, double b, double c, double d) {
     const bool pos = (a > 0.0) & (b > 0.0) & (c > 0.0) & (d > 0.0);
     const bool neg = (a < 0.0) & (b < 0.0) & (c < 0.0) & (d < 0.0);
-    const double mn = fmin(fmin(a, b), fmin(c, d));
-    const double mx = fmax(fmax(a, b), fmax(c, d));
+    const double mn = dmin(dmin(a, b), dmin(c, d));
+    const double mx = dmax(dmax(a, b), dmax(c, d));
     return pos ? mn : (neg ? mx : 0.0);
 }
 
 // O3 — REC: MP5 (Suresh & Huynh 1997) on POINT values.  Left-biased value at i+1/2
 // from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (S2).
-__device__ __noinline__ double mp5_limited(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
+// mp5_fast: the unlimited 5-point value and the S&H test; `need` is set when the limiter applies.
+__device__ __forceinline__ double mp5_fast(double vm2, double vm1, double v0, double vp1, double vp2, bool &need) {
+    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
+                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
+    const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
+    need = (vor - v0) * (vor - vmp) > 1e-10;
+    return vor;
+}
+// the limited value (slow path, out of line: it is rare on smooth data)
+__device__ __noinline__ double mp5_limited(double vm2, double vm1, double v0, double vp1, double vp2) {
     const double alpha = 4.0;
+    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
+                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
     const double dm1 = vm2 - 2.0 * vm1 + v0;
     const double d0 = vm1 - 2.0 * v0 + vp1;
     const double dp1 = v0 - 2.0 * vp1 + vp2;
@@ -49,17 +90,14 @@ __device__ __noinline__ double mp5_limited(double vm2, double vm1, double v0, do
     const double vav = 0.5 * (v0 + vp1);
     const double vmd = vav - 0.5 * dm4p;
     const double vlc = v0 + 0.5 * (v0 - vm1) + (4.0 / 3.0) * dm4m;
-    const double vmin = fmax(fmin(v0, fmin(vp1, vmd)), fmin(v0, fmin(vul, vlc)));
-    const double vmax = fmin(fmax(v0, fmax(vp1, vmd)), fmax(v0, fmax(vul, vlc)));
+    const double vmin = dmax(dmin(v0, dmin(vp1, vmd)), dmin(v0, dmin(vul, vlc)));
+    const double vmax = dmin(dmax(v0, dmax(vp1, vmd)), dmax(v0, dmax(vul, vlc)));
     return vor + minmod2(vmin - vor, vmax - vor);
 }
-
 __device__ __forceinline__ double mp5(double vm2, double vm1, double v0, double vp1, double vp2) {
-    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
-                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
-    const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
-    if ((vor - v0) * (vor - vmp) <= 1e-10) return vor;
-    return mp5_limited(vm2, vm1, v0, vp1, vp2, vor);
+    bool need;
+    const double vor = mp5_fast(vm2, vm1, v0, vp1, vp2, need);
+    return need ? mp5_limited(vm2, vm1, v0, vp1, vp2) : vor;
 }
 
 // ---------------------------------------------------------------- point physics
@@ -69,7 +107,7 @@ __device__ __forceinline__ void prim2cons(double gg, const double q[8], double u
     const double v2 = q[1] * q[1] + q[2] * q[2] + q[3] * q[3];
     const double B2 = q[5] * q[5] + q[6] * q[6] + q[7] * q[7];
     const double vB = q[1] * q[5] + q[2] * q[6] + q[3] * q[7];
-    const double W = rsqrt(1.0 - v2);
+    const double W = rsqrt_fast(1.0 - v2);
     const double y = (q[0] + gg * q[4]) * (W * W);
     const double yb = y + B2;
     u[0] = q[0] * W;
@@ -90,7 +128,7 @@ __device__ __forceinline__ void side_state(double gam, double gg, const double q
     const double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
     const double vB = v[0] * B[0] + v[1] * B[1] + v[2] * B[2];
     const double omv2 = 1.0 - v2;
-    const double W = rsqrt(omv2);
+    const double W = rsqrt_fast(omv2);
     const double rhoh = rho + gg * p;
     const double y = rhoh * (W * W);
     const double yb = y + B2;
@@ -111,15 +149,15 @@ __device__ __forceinline__ void side_state(double gam, double gg, const double q
     // O4: a^2 = cs^2 + ca^2 - cs^2 ca^2, cs^2 = gamma p/(rho h), ca^2 = b^2/(rho h + b^2)
     const double b2 = B2 * omv2 + vB * vB;
     const double w = rhoh + b2;
-    const double r = 1.0 / (rhoh * w);
+    const double r = rcp_fast(rhoh * w);
     const double cs2 = gam * p * w * r;
     const double ca2 = b2 * rhoh * r;
     const double a2 = cs2 + ca2 - cs2 * ca2;
     const double oma2 = 1.0 - a2;
     const double den = 1.0 - v2 * a2;
     const double vd = v[D];
-    const double root = sqrt(a2 * omv2 * (den - oma2 * vd * vd));
-    const double rden = 1.0 / den;
+    const double root = sqrt_fast(a2 * omv2 * (den - oma2 * vd * vd));
+    const double rden = rcp_fast(den);
     lp = (oma2 * vd + root) * rden;
     lm = (oma2 * vd - root) * rden;
 }
@@ -132,9 +170,9 @@ __device__ __forceinline__ void hll_face(double gam, double gg, const double qL[
     double uL[5], fL[5], uR[5], fR[5], lpL, lmL, lpR, lmR;
     side_state<D>(gam, gg, qL, uL, fL, lpL, lmL);
     side_state<D>(gam, gg, qR, uR, fR, lpR, lmR);
-    ap = fmax(0.0, fmax(lpL, lpR));
-    am = fmax(0.0, fmax(-lmL, -lmR));
-    const double inv = 1.0 / (ap + am);
+    ap = dmax(0.0, dmax(lpL, lpR));
+    am = dmax(0.0, dmax(-lmL, -lmR));
+    const double inv = rcp_fast(ap + am);
     const double wl = ap * inv, wr = am * inv, wd = ap * am * inv;
 #pragma unroll
     for (int c = 0; c < 5; ++c) F[c] = wl * fL[c] + wr * fR[c] - wd * (uR[c] - uL[c]);
@@ -146,24 +184,26 @@ __device__ __forceinline__ void hll_face(double gam, double gg, const double qL[
 // ---------------------------------------------------------------- O2: con2prim
 // Newton on y = rho h W^2 from the upper bound y0 = gamma (U - B^2/2); safeguard and stopping
 // rule as in DESIGN.md O2.  Returns the number of Newton updates (>=1) or -(count) on failure.
-struct C2PEval { double x, p, f, df; };
+struct C2PEval { double x, sq, p, f, df; };
 
 __device__ __forceinline__ bool c2p_eval(double g1, double D, double S2, double B2, double T, double U, double y,
                                          C2PEval &a) {
     if (!(y > 0.0) || !isfinite(y)) return false;
     const double yb = y + B2;
     const double y2 = y * y, yb2 = yb * yb;
-    const double r = 1.0 / (y2 * y * yb2 * yb);   // 1/(y^3 (y+B^2)^3)
+    const double r = rcp_fast(y2 * y * yb2 * yb);   // 1/(y^3 (y+B^2)^3)
     const double x = (S2 * y2 + T * (2.0 * y + B2)) * (y * yb) * r;
     if (!(x < 1.0) || !(x >= 0.0)) return false;
     const double omx = 1.0 - x;
-    const double sq = sqrt(omx);
+    const double rsq = rsqrt_fast(omx);
+    const double sq = omx * rsq;
     const double xp = -2.0 * (S2 * y2 * y + T * (3.0 * y2 + 3.0 * y * B2 + B2 * B2)) * r;
     const double Ty3 = T * (yb2 * yb) * r;        // T / y^3
     a.x = x;
+    a.sq = sq;
     a.p = g1 * (y * omx - D * sq);
     a.f = y - a.p + 0.5 * (1.0 + x) * B2 - 0.5 * Ty3 * y - U;
-    a.df = 1.0 - g1 * omx - g1 * (-y + 0.5 * D / sq) * xp + 0.5 * B2 * xp + Ty3;
+    a.df = 1.0 - g1 * omx - g1 * (-y + 0.5 * D * rsq) * xp + 0.5 * B2 * xp + Ty3;
     return true;
 }
 
@@ -190,7 +230,7 @@ __device__ __forceinline__ int con2prim(double gam, const double u[5], const dou
             continue;
         }
         ylast = y;
-        const double dy = -a.f / a.df;
+        const double dy = -a.f * rcp_fast(a.df);
         y = y + dy;
         ++it;
         if (fabs(dy) <= tol * fabs(y)) { conv = true; break; }
@@ -200,10 +240,10 @@ __device__ __forceinline__ int con2prim(double gam, const double u[5], const dou
         q[0] = q[1] = q[2] = q[3] = q[4] = nan;
         return -(it > 0 ? it : 1);
     }
-    q[0] = D * sqrt(1.0 - a.x);
+    q[0] = D * a.sq;
     q[4] = a.p;
-    const double ryb = 1.0 / (y + B2);
-    const double sby = SB / y;
+    const double ryb = rcp_fast(y + B2);
+    const double sby = SB * rcp_fast(y);
     q[1] = (u[1] + sby * B[0]) * ryb;
     q[2] = (u[2] + sby * B[1]) * ryb;
     q[3] = (u[3] + sby * B[2]) * ryb;

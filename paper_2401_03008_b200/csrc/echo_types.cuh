@@ -7,7 +7,7 @@ namespace echo {
 // Grid geometry: unit periodic box, h_d = 1/n_d, x fastest.
 struct Grid {
     int n[3];
-    long long s[3];   // linear strides: 1, nx, nx*ny
+    int s[3];         // linear strides in elements: 1, nx, nx*ny (N < 2^31: 32-bit cell indices)
     long long N;
     double h[3], rh[3];   // spacing and its reciprocal (n_d exactly)
 };
