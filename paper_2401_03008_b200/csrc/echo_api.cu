@@ -57,7 +57,7 @@ int cuda_fail(echo_ctx *c, cudaError_t e, const char *where) {
     } while (0)
 
 // flux-sweep tiling: threads per block, transverse width, max tile length
-constexpr int FLUX_NT = 128, FLUX_TX = 4, FLUX_TYZ = 16, FLUX_LX = 64, FLUX_LYZ = 64;
+constexpr int FLUX_NT = 128, FLUX_CMAX = 512;
 
 enum { KC_PRIM = 0, KC_FLUX = 1, KC_UCT = 4, KC_UPDATE = 5, KC_CTRL = 6, KC_OTHER = 7 };
 
@@ -108,16 +108,14 @@ Stage make_stage(const echo_ctx *c, int which) {
 
 template <int D>
 int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax) {
-    constexpr int NT = FLUX_NT, T = (D == 0) ? FLUX_TX : FLUX_TYZ;
+    constexpr int NT = FLUX_NT, T = (D == 0) ? 4 : 16;
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
-    const int Lmax = (D == 0) ? FLUX_LX : FLUX_LYZ;
-    const int tilesD = (g.n[D] + Lmax - 1) / Lmax;
-    const int L = (g.n[D] + tilesD - 1) / tilesD;
-    const int tilesT = (g.n[TD] + T - 1) / T;
-    const size_t smem = sizeof(double) * 5 * (size_t)(L + 5) * T;
-    dim3 grid(tilesT, tilesD, g.n[OD]);
-    KL(KC_FLUX + D, "k_flux", k_flux<D, T, NT><<<grid, NT, smem, ctx->stream>>>(g, st, L, ctx->gamma, ctx->gg, ctx->ctrl, want_amax));
+    // chunks along D: one chunk per column unless the axis is long (5 halo faces per chunk are recomputed)
+    const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
+    const int C = (g.n[D] + nchunk - 1) / nchunk;
+    dim3 grid((g.n[TD] + T - 1) / T, nchunk, g.n[OD]);
+    KL(KC_FLUX + D, "k_flux", k_flux<D, NT><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax));
     return ECHO_OK;
 }
 
@@ -206,9 +204,6 @@ int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     h.one = 1;
     CU(cudaMemcpyAsync(ctx->ctrl, &h, sizeof(h), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));   // h is a stack object
-    CU(cudaFuncSetAttribute(k_flux<0, FLUX_TX, FLUX_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-    CU(cudaFuncSetAttribute(k_flux<1, FLUX_TYZ, FLUX_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-    CU(cudaFuncSetAttribute(k_flux<2, FLUX_TYZ, FLUX_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
     ctx->bound = true;
     ctx->has_state = false;
     return ECHO_OK;

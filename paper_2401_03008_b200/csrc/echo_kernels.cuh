@@ -133,87 +133,149 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
 }
 
 // ------------------------------------------------------------------ points 2+3: fused flux sweep
-// Direction D.  A block owns a tile of L cells along D times T cells along the contiguous
-// transverse axis TD (y for the x-sweep, x otherwise) at one coordinate of the remaining axis.
-// Phase 1: the L+5 face fluxes F_{m0-3 .. m0+L+1} (5 components) go to shared memory; faces
-// m0..m0+L-1 also store a+, a-, vbar and feed the a_max reduction.
-// Phase 2: rhs -= (F^_{i+1/2} - F^_{i-1/2})/h_D from shared memory (DER).  The 5 halo
-// faces are recomputed by the neighbouring tile with the same instructions on the same inputs,
-// hence bit-identically: conservation stays at round-off.
+// Direction D.  A block owns T cells along the transverse axis TD (y for the x-sweep, x otherwise)
+// at one coordinate of the remaining axis and MARCHES along D over a chunk of C cells, R = NT/T
+// face-rows per round, through two shared-memory rings of 3R rows:
+//   prim ring: the 8 input fields (rho, v, p, 2 transverse centred B, normal staggered B), filled
+//              by cp.async (LDGSTS) one group of R rows two rounds ahead of its use, with the
+//              periodic wrap applied to the source row; the global-memory latency is hidden behind
+//              the arithmetic of the two rounds in between and costs no registers;
+//   F ring:    the 5 HLL flux components of the last 3R faces.
+// Round t: (1) wait for the copies, one __syncthreads; (2) prefetch group t+2; (3) DER + flux
+// difference (O6) for the R cells whose six faces are complete (lagging 5 rows); (4) faces
+// R t .. R t + R-1: MP5 L/R states (O3), HLL (O5), store a+, a-, vbar, a_max.
+// Only the first 5 faces of a chunk are recomputed by the neighbouring chunk (with the same
+// instructions on the same inputs, hence bit-identically: conservation stays at round-off).
 // REC: all 14 unlimited MP5 values and their S&H tests first; the limiter itself runs out of line
 // only for the (field, side) pairs whose test fired (never on smooth data).
-template <int D, int T, int NT>
-__global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int L, double gam, double gg, Ctrl *ctrl,
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int D, int NT>
+__global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
                                              int want_amax) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
     constexpr int OD = 3 - D - TD;            // remaining axis
     constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
-    extern __shared__ double sF[];
-    const int LA = L + 5;
-    const int m0 = blockIdx.y * L;
-    const int t0 = blockIdx.x * T;
+    constexpr int T = (D == 0) ? 4 : 16;      // tile width along TD
+    constexpr int R = NT / T;                 // face-rows per round
+    constexpr int RL = 3 * R;                 // ring length (rows)
+    // shared-memory strides in elements.  x-sweep: [field][b][row] with the b-stride padded to
+    // 4 mod 16 so that a warp's 8 rows x 4 b fall in distinct banks; y/z: [row][field][b].
+    constexpr int SB = (D == 0) ? RL + 4 : 1;
+    constexpr int SR = (D == 0) ? 1 : 8 * T;
+    constexpr int SV = (D == 0) ? T * SB : T;
+    constexpr int FR = (D == 0) ? 1 : 5 * T;
+    constexpr int FV = SV;
+    __shared__ double sP[(D == 0) ? 8 * T * SB : RL * 8 * T];
+    __shared__ double sF[(D == 0) ? 5 * T * SB : RL * 5 * T];
+
     const int nD = g.n[D], nT = g.n[TD];
-    const int Lv = min(L, nD - m0);           // valid cells of this tile along D
+    const int m0 = blockIdx.y * C;
+    const int Cv = min(C, nD - m0);           // cells of this chunk
+    const int t0 = blockIdx.x * T;
     const int sD = g.s[D], sT = g.s[TD];
     const int baseO = g.s[OD] * (int)blockIdx.z;
-    const int nface = LA * T;
+    const int tid = threadIdx.x;
+
+    // ---- global -> shared copy mapping (lanes along the contiguous global axis)
+    const int la = (D == 0) ? tid % R : tid / T;
+    const int lb = (D == 0) ? tid / R : tid % T;
+    const int lsrc = baseO + sT * min(t0 + lb, nT - 1);
+    const double *fld[8] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2], st.Bf[D]};
+    auto issue = [&](int grp) {
+        const int src = lsrc + sD * wrapi(m0 - 5 + R * grp + la, nD);
+        double *dst = sP + ((grp % 3) * R + la) * SR + lb * SB;
+#pragma unroll
+        for (int v = 0; v < 8; ++v) cp_async8(dst + v * SV, fld[v] + src);
+        cp_async_commit();
+    };
+
+    // ---- compute mapping
+    const int a = tid / T, b = tid % T;
+    const bool colok = (t0 + b) < nT;
+    const int ocol = baseO + sT * (t0 + b);
+    const int nfr = Cv + 5;                   // face-rows m0-3 .. m0+Cv+1
+    const int nround = (nfr + R - 1) / R;
+    const double mrh = -g.rh[D];
     double amax = 0.0;
 
-    // face slot f -> (a along D, b along TD); lanes run along the contiguous axis
-    int a, b;
-    if (D == 0) { a = threadIdx.x % LA; b = threadIdx.x / LA; } else { b = threadIdx.x % T; a = threadIdx.x / T; }
-    for (int f = threadIdx.x; f < nface; f += NT) {
-        const int cT = t0 + b;
-        if (cT < nT && a < Lv + 5) {
-            const int m = m0 - 3 + a;             // face m sits between cells m and m+1
-            const int base = baseO + sT * cT;
-            int idx[6];
+    issue(0);
+    issue(1);
+    for (int t = 0; t <= nround; ++t) {
+        cp_async_wait_all();
+        __syncthreads();
+        if (t + 2 <= nround) issue(t + 2);
+
+        // (3) DER + divergence of the cells completed by round t-1
+        if (t >= 1) {
+            const int i = R * (t - 1) - 5 + a;            // cell row within the chunk
+            if (colok && i >= 0 && i < Cv) {
+                int sl[6];
+                int r0 = ((t - 1) % 3) * R - 5 + a;
+                if (r0 < 0) r0 += RL;
 #pragma unroll
-            for (int s = 0; s < 6; ++s) idx[s] = base + sD * wrapi(m - 2 + s, nD);
+                for (int k = 0; k < 6; ++k) { sl[k] = r0 * FR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
+                const int o = ocol + sD * (m0 + i);
+                const double *Fb = sF + b * SB;
+#pragma unroll
+                for (int c = 0; c < 5; ++c) {
+                    const double *F = Fb + c * FV;
+                    const double r = mrh * der_diff(F[sl[0]], F[sl[1]], F[sl[2]], F[sl[3]], F[sl[4]], F[sl[5]]);
+                    if (D == 0) st.R[c][o] = r; else st.R[c][o] += r;
+                }
+            }
+        }
+
+        // (4) the faces of round t
+        const int f = R * t + a;
+        if (t < nround && colok && f < nfr) {
+            int sl[6];
+            int r0 = (t % 3) * R + a;
+            const int fslot = r0 * FR;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) { sl[k] = r0 * SR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
+            const double *Pb = sP + b * SB;
             double qL[8], qR[8];
             unsigned need = 0u;
-            {
-                const double *rec[7] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2]};
-                const int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+            constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
 #pragma unroll
-                for (int v = 0; v < 7; ++v) {
-                    double s[6];
-#pragma unroll
-                    for (int k = 0; k < 6; ++k) s[k] = __ldg(rec[v] + idx[k]);
-                    bool nl, nr;
-                    qL[slot[v]] = mp5_fast(s[0], s[1], s[2], s[3], s[4], nl);
-                    qR[slot[v]] = mp5_fast(s[5], s[4], s[3], s[2], s[1], nr);
-                    need |= (nl ? 1u : 0u) << (2 * v) | (nr ? 1u : 0u) << (2 * v + 1);
-                }
-                if (need) {
+            for (int v = 0; v < 7; ++v) {
+                const double *p = Pb + v * SV;
+                const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
+                bool nl, nr;
+                qL[slot[v]] = mp5_fast(s0, s1, s2, s3, s4, nl);
+                qR[slot[v]] = mp5_fast(s5, s4, s3, s2, s1, nr);
+                need |= (nl ? 1u : 0u) << (2 * v) | (nr ? 1u : 0u) << (2 * v + 1);
+            }
+            if (need) {
 #pragma unroll 1
-                    for (int v = 0; v < 7; ++v) {
-                        const unsigned bits = (need >> (2 * v)) & 3u;
-                        if (!bits) continue;
-                        const double *fp = rec[0];
+                for (int v = 0; v < 7; ++v) {
+                    const unsigned bits = (need >> (2 * v)) & 3u;
+                    if (!bits) continue;
+                    const double *p = Pb + v * SV;
+                    const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
+                    const double lim_l = (bits & 1u) ? mp5_limited(s0, s1, s2, s3, s4) : 0.0;
+                    const double lim_r = (bits & 2u) ? mp5_limited(s5, s4, s3, s2, s1) : 0.0;
 #pragma unroll
-                        for (int w = 1; w < 7; ++w) fp = (v == w) ? rec[w] : fp;
-                        double s[6];
-#pragma unroll
-                        for (int k = 0; k < 6; ++k) s[k] = __ldg(fp + idx[k]);
-                        const double lim_l = (bits & 1u) ? mp5_limited(s[0], s[1], s[2], s[3], s[4]) : 0.0;
-                        const double lim_r = (bits & 2u) ? mp5_limited(s[5], s[4], s[3], s[2], s[1]) : 0.0;
-#pragma unroll
-                        for (int w = 0; w < 7; ++w) {
-                            if (w == v && (bits & 1u)) qL[slot[w]] = lim_l;
-                            if (w == v && (bits & 2u)) qR[slot[w]] = lim_r;
-                        }
+                    for (int w = 0; w < 7; ++w) {
+                        if (w == v && (bits & 1u)) qL[slot[w]] = lim_l;
+                        if (w == v && (bits & 2u)) qR[slot[w]] = lim_r;
                     }
                 }
             }
-            qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + idx[2]);   // the normal B is the staggered value
+            qL[5 + D] = qR[5 + D] = Pb[7 * SV + sl[2]];   // the normal B is the staggered value
             double F[5], ap, am, vb1, vb2;
             hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
-            const int so = (D == 0) ? (b * LA + a) : (a * T + b);
+            double *Fo = sF + b * SB + fslot;
 #pragma unroll
-            for (int c = 0; c < 5; ++c) sF[c * nface + so] = F[c];
-            if (a >= 3 && a < Lv + 3) {
-                const int o = idx[2];
+            for (int c = 0; c < 5; ++c) Fo[c * FV] = F[c];
+            if (f >= 3 && f < Cv + 3) {
+                const int o = ocol + sD * (m0 + f - 3);
                 st.ap[D][o] = ap;
                 st.am[D][o] = am;
                 st.vb[D][0][o] = vb1;
@@ -221,37 +283,15 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int L, double gam
                 amax = dmax(amax, dmax(ap, am));
             }
         }
-        if (D == 0) { a += NT; while (a >= LA) { a -= LA; ++b; } } else { a += NT / T; }
-    }
-    __syncthreads();
-
-    const double mrh = -g.rh[D];
-    const int ncell = L * T;
-    if (D == 0) { a = threadIdx.x % L; b = threadIdx.x / L; } else { b = threadIdx.x % T; a = threadIdx.x / T; }
-    for (int e = threadIdx.x; e < ncell; e += NT) {
-        const int cT = t0 + b;
-        if (cT < nT && a < Lv) {
-            const int o = baseO + sT * cT + sD * (m0 + a);
-            constexpr int one = 1;
-            const int step = (D == 0) ? one : T;
-            const int so = (D == 0) ? (b * LA + a) : (a * T + b);
-#pragma unroll
-            for (int c = 0; c < 5; ++c) {
-                const double *F = sF + c * nface + so;
-                const double r = mrh * der_diff(F[0], F[step], F[2 * step], F[3 * step], F[4 * step], F[5 * step]);
-                if (D == 0) st.R[c][o] = r; else st.R[c][o] += r;
-            }
-        }
-        if (D == 0) { a += NT; while (a >= L) { a -= L; ++b; } } else { a += NT / T; }
     }
 
     if (want_amax) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) amax = dmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
         __shared__ double wmax[NT / 32];
-        if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = amax;
+        if ((tid & 31) == 0) wmax[tid >> 5] = amax;
         __syncthreads();
-        if (threadIdx.x == 0) {
+        if (tid == 0) {
             double m = wmax[0];
 #pragma unroll
             for (int w = 1; w < NT / 32; ++w) m = dmax(m, wmax[w]);
