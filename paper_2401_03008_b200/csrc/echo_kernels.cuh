@@ -146,8 +146,8 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
 // R t .. R t + R-1: MP5 L/R states (O3), HLL (O5), store a+, a-, vbar, a_max.
 // Only the first 5 faces of a chunk are recomputed by the neighbouring chunk (with the same
 // instructions on the same inputs, hence bit-identically: conservation stays at round-off).
-// REC: all 14 unlimited MP5 values and their S&H tests first; the limiter itself runs out of line
-// only for the (field, side) pairs whose test fired (never on smooth data).
+// REC: the unlimited MP5 value and the S&H test; the limiter proper runs (inline branch) only where
+// the test fires, which on the smooth wave is the couple of cells around each extremum.
 __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
@@ -241,32 +241,13 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam
             for (int k = 0; k < 6; ++k) { sl[k] = r0 * SR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
             const double *Pb = sP + b * SB;
             double qL[8], qR[8];
-            unsigned need = 0u;
             constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
 #pragma unroll
             for (int v = 0; v < 7; ++v) {
                 const double *p = Pb + v * SV;
                 const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
-                bool nl, nr;
-                qL[slot[v]] = mp5_fast(s0, s1, s2, s3, s4, nl);
-                qR[slot[v]] = mp5_fast(s5, s4, s3, s2, s1, nr);
-                need |= (nl ? 1u : 0u) << (2 * v) | (nr ? 1u : 0u) << (2 * v + 1);
-            }
-            if (need) {
-#pragma unroll 1
-                for (int v = 0; v < 7; ++v) {
-                    const unsigned bits = (need >> (2 * v)) & 3u;
-                    if (!bits) continue;
-                    const double *p = Pb + v * SV;
-                    const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
-                    const double lim_l = (bits & 1u) ? mp5_limited(s0, s1, s2, s3, s4) : 0.0;
-                    const double lim_r = (bits & 2u) ? mp5_limited(s5, s4, s3, s2, s1) : 0.0;
-#pragma unroll
-                    for (int w = 0; w < 7; ++w) {
-                        if (w == v && (bits & 1u)) qL[slot[w]] = lim_l;
-                        if (w == v && (bits & 2u)) qR[slot[w]] = lim_r;
-                    }
-                }
+                qL[slot[v]] = mp5(s0, s1, s2, s3, s4);
+                qR[slot[v]] = mp5(s5, s4, s3, s2, s1);
             }
             qL[5 + D] = qR[5 + D] = Pb[7 * SV + sl[2]];   // the normal B is the staggered value
             double F[5], ap, am, vb1, vb2;
@@ -313,37 +294,14 @@ __device__ __forceinline__ double uct_edge(const Stage &st, const int (*ix)[6], 
     // q = 0: vbar_i along i, 1: B_j along i, 2: vbar_j along j, 3: B_i along j
     const double *fld[4] = {st.vb[J][1], st.Bf[J], st.vb[I][0], st.Bf[I]};
     double L[4], R[4];
-    unsigned need = 0u;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         const int *x = ix[q < 2 ? I : J];
         double s[6];
 #pragma unroll
         for (int m = 0; m < 6; ++m) s[m] = __ldg(fld[q] + x[m]);
-        bool nl, nr;
-        L[q] = mp5_fast(s[0], s[1], s[2], s[3], s[4], nl);
-        R[q] = mp5_fast(s[5], s[4], s[3], s[2], s[1], nr);
-        need |= (nl ? 1u : 0u) << (2 * q) | (nr ? 1u : 0u) << (2 * q + 1);
-    }
-    if (need) {
-#pragma unroll 1
-        for (int q = 0; q < 4; ++q) {
-            const unsigned bits = (need >> (2 * q)) & 3u;
-            if (!bits) continue;
-            const double *fp = fld[0];
-#pragma unroll
-            for (int w = 1; w < 4; ++w) fp = (q == w) ? fld[w] : fp;
-            double s[6];
-#pragma unroll
-            for (int m = 0; m < 6; ++m) s[m] = __ldg(fp + (q < 2 ? ix[I][m] : ix[J][m]));
-            const double lim_l = (bits & 1u) ? mp5_limited(s[0], s[1], s[2], s[3], s[4]) : 0.0;
-            const double lim_r = (bits & 2u) ? mp5_limited(s[5], s[4], s[3], s[2], s[1]) : 0.0;
-#pragma unroll
-            for (int w = 0; w < 4; ++w) {
-                if (w == q && (bits & 1u)) L[w] = lim_l;
-                if (w == q && (bits & 2u)) R[w] = lim_r;
-            }
-        }
+        L[q] = mp5(s[0], s[1], s[2], s[3], s[4]);
+        R[q] = mp5(s[5], s[4], s[3], s[2], s[1]);
     }
     const int cj = ix[J][3], ci = ix[I][3];   // neighbours +1 along j and along i
     const double aip = dmax(__ldg(st.ap[I] + c), __ldg(st.ap[I] + cj));

@@ -59,45 +59,52 @@ __device__ __forceinline__ double minmod2(double a, double b) {
     return ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
 }
 __device__ __forceinline__ double minmod4(double a, double b, double c, double d) {
-    const bool pos = (a > 0.0) & (b > 0.0) & (c > 0.0) & (d > 0.0);
-    const bool neg = (a < 0.0) & (b < 0.0) & (c < 0.0) & (d < 0.0);
-    const double mn = dmin(dmin(a, b), dmin(c, d));
-    const double mx = dmax(dmax(a, b), dmax(c, d));
-    return pos ? mn : (neg ? mx : 0.0);
+    // all four of one sign: the one of smallest magnitude; else 0.  Sign agreement on the high
+    // words (integer pipe); the magnitude minimum with |.| operand modifiers (3 DSETP).  A zero
+    // argument makes the magnitude minimum 0, so its sign bit does not matter.
+    const int ha = __double2hiint(a);
+    const int diff = (ha ^ __double2hiint(b)) | (ha ^ __double2hiint(c)) | (ha ^ __double2hiint(d));
+    double m = (fabs(a) < fabs(b)) ? a : b;
+    m = (fabs(m) < fabs(c)) ? m : c;
+    m = (fabs(m) < fabs(d)) ? m : d;
+    return diff >= 0 ? m : 0.0;
 }
 
 // O3 — REC: MP5 (Suresh & Huynh 1997) on POINT values.  Left-biased value at i+1/2
-// from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (S2).
-// mp5_fast: the unlimited 5-point value and the S&H test; `need` is set when the limiter applies.
-__device__ __forceinline__ double mp5_fast(double vm2, double vm1, double v0, double vp1, double vp2, bool &need) {
-    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
-                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
-    const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
-    need = (vor - v0) * (vor - vmp) > 1e-10;
-    return vor;
-}
-// the limited value (slow path, out of line: it is rare on smooth data)
-__device__ __noinline__ double mp5_limited(double vm2, double vm1, double v0, double vp1, double vp2) {
-    const double alpha = 4.0;
-    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
-                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
-    const double dm1 = vm2 - 2.0 * vm1 + v0;
-    const double d0 = vm1 - 2.0 * v0 + vp1;
-    const double dp1 = v0 - 2.0 * vp1 + vp2;
-    const double dm4p = minmod4(4.0 * d0 - dp1, 4.0 * dp1 - d0, d0, dp1);
-    const double dm4m = minmod4(4.0 * dm1 - d0, 4.0 * d0 - dm1, dm1, d0);
-    const double vul = v0 + alpha * (v0 - vm1);
-    const double vav = 0.5 * (v0 + vp1);
-    const double vmd = vav - 0.5 * dm4p;
-    const double vlc = v0 + 0.5 * (v0 - vm1) + (4.0 / 3.0) * dm4m;
-    const double vmin = dmax(dmin(v0, dmin(vp1, vmd)), dmin(v0, dmin(vul, vlc)));
-    const double vmax = dmin(dmax(v0, dmax(vp1, vmd)), dmax(v0, dmax(vul, vlc)));
+// from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (S2).  The unlimited 5-point value and the S&H test
+// come first; the limiter proper is evaluated (inline, branch) only where the test fires: on smooth
+// data that is the few cells around each extremum.
+__device__ __forceinline__ double mp5_limit(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
+    const double dm1 = fma(-2.0, vm1, vm2) + v0;
+    const double d0 = fma(-2.0, v0, vm1) + vp1;
+    const double dp1 = fma(-2.0, vp1, v0) + vp2;
+    const double dm4p = minmod4(fma(4.0, d0, -dp1), fma(4.0, dp1, -d0), d0, dp1);
+    const double dm4m = minmod4(fma(4.0, dm1, -d0), fma(4.0, d0, -dm1), dm1, d0);
+    const double dv = v0 - vm1;
+    const double vul = fma(4.0, dv, v0);
+    const double vmd = fma(0.5, v0 + vp1, -0.5 * dm4p);
+    const double vlc = fma(0.5, dv, v0) + (4.0 / 3.0) * dm4m;
+    // min/max of (v0, vp1, vmd) and of (v0, vul, vlc), sharing the comparisons
+    const bool c1 = v0 < vp1;
+    const double lo1 = c1 ? v0 : vp1, hi1 = c1 ? vp1 : v0;
+    const double mn1 = dmin(lo1, vmd), mx1 = dmax(hi1, vmd);
+    const bool c2 = v0 < vul;
+    const double lo2 = c2 ? v0 : vul, hi2 = c2 ? vul : v0;
+    const double mn2 = dmin(lo2, vlc), mx2 = dmax(hi2, vlc);
+    const double vmin = dmax(mn1, mn2);
+    const double vmax = dmin(mx1, mx2);
     return vor + minmod2(vmin - vor, vmax - vor);
 }
 __device__ __forceinline__ double mp5(double vm2, double vm1, double v0, double vp1, double vp2) {
-    bool need;
-    const double vor = mp5_fast(vm2, vm1, v0, vp1, vp2, need);
-    return need ? mp5_limited(vm2, vm1, v0, vp1, vp2) : vor;
+    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
+                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
+    const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
+    double r = vor;
+    if ((vor - v0) * (vor - vmp) > 1e-10) {
+        asm volatile("" ::: "memory");   // keeps this a real branch: the limiter must not be if-converted
+        r = mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
+    }
+    return r;
 }
 
 // ---------------------------------------------------------------- point physics
