@@ -106,8 +106,9 @@ Stage make_stage(const echo_ctx *c, int which) {
     return st;
 }
 
-template <int D>
-int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax) {
+// fuse: 0 = plain operator (rhs written), 1 = the z-sweep applies the RK combination of the 5 cell fields
+template <int D, int MODE>
+int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu) {
     constexpr int NT = FLUX_NT, T = (D == 0) ? 4 : 16;
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
@@ -115,26 +116,49 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax) {
     const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
     const int C = (g.n[D] + nchunk - 1) / nchunk;
     dim3 grid((g.n[TD] + T - 1) / T, nchunk, g.n[OD]);
-    KL(KC_FLUX + D, "k_flux", k_flux<D, NT><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax));
+    KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
     return ECHO_OK;
 }
 
+// RK bookkeeping of one stage inside echo_step: which buffers hold what
+struct StagePlan {
+    bool prim_upd;      // k_prim first forms U1 = U^n + dt*R (the deferred stage-1 update) and stores it
+    bool fuse_z;        // the z-sweep applies out = c0*U^n + c1*(cur + dt*rhs) to the 5 cell fields
+    int cur, out;       // 0 = U^n buffers, 1 = stage buffers
+    double c0, c1;
+};
+
 // points 1-4 of a sub-step on the given stage pointers
-int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax) {
+int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan *pl = nullptr) {
     const Grid &g = ctx->g;
-    KL(KC_PRIM, "k_prim", k_prim<false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
+    PrimUpd pu;
+    for (int v = 0; v < 5; ++v) pu.uout[v] = ctx->field[F_U1 + v];
+    if (pl && pl->prim_upd)
+        KL(KC_PRIM, "k_prim", k_prim<false, true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+    else
+        KL(KC_PRIM, "k_prim", k_prim<false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+    FluxUpd fu;
+    for (int v = 0; v < 5; ++v) {
+        fu.base[v] = ctx->field[F_U + v];
+        fu.cur[v] = ctx->field[((pl && pl->cur) ? F_U1 : F_U) + v];
+        fu.out[v] = ctx->field[((pl && pl->out) ? F_U1 : F_U) + v];
+    }
+    fu.c0 = pl ? pl->c0 : 0.0;
+    fu.c1 = pl ? pl->c1 : 1.0;
     int rc;
-    if ((rc = launch_flux<0>(ctx, st, want_amax))) return rc;
-    if ((rc = launch_flux<1>(ctx, st, want_amax))) return rc;
-    if ((rc = launch_flux<2>(ctx, st, want_amax))) return rc;
-    if (want_amax == 2) {   // stage 1 of echo_step: dt must exist before the update (S9)
+    if ((rc = launch_flux<0, 0>(ctx, st, want_amax, fu))) return rc;
+    if ((rc = launch_flux<1, 0>(ctx, st, want_amax, fu))) return rc;
+    if (pl && pl->fuse_z) { if ((rc = launch_flux<2, 1>(ctx, st, want_amax, fu))) return rc; }
+    else                  { if ((rc = launch_flux<2, 0>(ctx, st, want_amax, fu))) return rc; }
+    if (want_amax == 2) {   // stage 1 of echo_step: dt must exist before any update (S9)
         KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
     }
     KL(KC_UCT, "k_uct", k_uct<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st));
     return ECHO_OK;
 }
 
-int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, double c0, double c1) {
+// curl + RK combination of the staggered B (and, with_u, of the 5 cell fields as well)
+int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, double c0, double c1, bool with_u) {
     Update up;
     for (int v = 0; v < 8; ++v) {
         up.base[v] = ctx->field[F_U + v];
@@ -144,8 +168,12 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
     up.c0 = c0;
     up.c1 = c1;
     const Grid &g = ctx->g;
-    KL(KC_UPDATE, "k_update", k_update<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1], st.R[2],
-                                                             st.R[3], st.R[4], up, ctx->ctrl, 1));
+    if (with_u)
+        KL(KC_UPDATE, "k_update", k_update<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1],
+                                                                              st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
+    else
+        KL(KC_UPDATE, "k_update", k_update<false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1],
+                                                                               st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
     return ECHO_OK;
 }
 
@@ -263,15 +291,24 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     for (int n = 0; n < nsteps; ++n) {
         KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
-        // stage 1: U1 = U^n + dt L(U^n), dt from the speeds of this very operator (S9)
+        // stage 1: L(U^n), dt from its speeds (S9); B1 = B^n + dt rhs_B now, U1 = U^n + dt rhs_U deferred
+        // into the k_prim of stage 2 (st.U = U^n, st.R = rhs, result stored to the stage buffers)
         if ((rc = launch_operator(ctx, s0, 2))) return rc;
-        if ((rc = launch_update(ctx, s0, 0, 1, 0.0, 1.0))) return rc;
-        // stage 2: U2 = 3/4 U^n + 1/4 (U1 + dt L(U1))
-        if ((rc = launch_operator(ctx, s1, 0))) return rc;
-        if ((rc = launch_update(ctx, s1, 1, 1, 0.75, 0.25))) return rc;
+        if ((rc = launch_update(ctx, s0, 0, 1, 0.0, 1.0, false))) return rc;
+        // stage 2: U2 = 3/4 U^n + 1/4 (U1 + dt L(U1)); the cell fields are combined inside the z-sweep
+        {
+            Stage s12 = s1;                       // operator state: faces from the stage buffers ...
+            for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];   // ... cell fields = U^n (+ dt R inside k_prim)
+            const StagePlan pl = {true, true, 1, 1, 0.75, 0.25};
+            if ((rc = launch_operator(ctx, s12, 0, &pl))) return rc;
+            if ((rc = launch_update(ctx, s1, 1, 1, 0.75, 0.25, false))) return rc;
+        }
         // stage 3: U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
-        if ((rc = launch_operator(ctx, s1, 0))) return rc;
-        if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0))) return rc;
+        {
+            const StagePlan pl = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
+            if ((rc = launch_operator(ctx, s1, 0, &pl))) return rc;
+            if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false))) return rc;
+        }
         KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
     }
     return ECHO_OK;
@@ -287,7 +324,7 @@ int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, doub
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 5; ++v) st.P[v] = out[v];
     for (int d = 0; d < 3; ++d) st.Bc[d] = out[5 + d];
-    KL(KC_PRIM, "k_prim", k_prim<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
+    KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
     double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d)
         if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -302,7 +339,7 @@ int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy,
     const Grid &g = ctx->g;
     const size_t nb = sizeof(double) * g.N;
     Stage st = make_stage(ctx, 0);
-    KL(KC_PRIM, "k_prim", k_prim<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
+    KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 8; ++v) CU(cudaMemcpyAsync(out[v], ctx->field[F_P + v], nb, cudaMemcpyDeviceToHost, ctx->stream));
     double *bf[3] = {bxf, byf, bzf};
@@ -399,7 +436,7 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
                                            f + 7 * np, ctx->part));
     Stage st = make_stage(ctx, 0);
     KL(KC_CTRL, "k_c2p_stats_reset", k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
-    KL(KC_PRIM, "k_prim", k_prim<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl));
+    KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
     KL(KC_OTHER, "k_extrema", k_extrema<<<NPART, 256, 0, ctx->stream>>>(g.N, st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], ctx->part));
     double dmax = 0.0;
     if ((rc = echo_div_b(ctx, nullptr, &dmax))) return rc;   // synchronises

@@ -55,8 +55,14 @@ __global__ void k_c2p_stats_reset(Ctrl *c) {
 // inside echo_step only failures are counted (no atomics at all on healthy data).
 // Divergent Newton counts: each lane runs its own loop and freezes at its own convergence, so a
 // cell's result never depends on which cells share its warp (translation covariance stays bitwise).
-template <bool STATS>
-__global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl) {
+// UPD: the stage-1 Runge-Kutta update of the conserved cell fields, U1 = U^n + dt L(U^n) (O9), is done
+// here, on the fly, by the INT+con2prim pass of stage 2 (st.U = U^n, st.R = L(U^n), result stored to
+// uout and inverted at once): dt only exists after all three stage-1 sweeps, and this kernel has
+// spare memory bandwidth, so the update costs no pass of its own and U1 is never re-read.
+struct PrimUpd { double *uout[5]; };
+
+template <bool STATS, bool UPD>
+__global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
@@ -74,8 +80,16 @@ __global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl
             for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
             B[d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
         }
-        const double u[5] = {__ldg(st.U[0] + c), __ldg(st.U[1] + c), __ldg(st.U[2] + c), __ldg(st.U[3] + c),
-                             __ldg(st.U[4] + c)};
+        double u[5] = {__ldg(st.U[0] + c), __ldg(st.U[1] + c), __ldg(st.U[2] + c), __ldg(st.U[3] + c),
+                       __ldg(st.U[4] + c)};
+        if (UPD) {
+            const double dt = ctrl->dt;
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                u[v] = u[v] + dt * __ldg(st.R[v] + c);
+                pu.uout[v][c] = u[v];
+            }
+        }
         double q[5];
         it = con2prim(gam, u, B, q);
 #pragma unroll
@@ -155,9 +169,16 @@ __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int D, int NT>
+// MODE 0: rhs is written (x) or accumulated (y, z).  MODE 1 (last sweep of RK stages 2 and 3): the
+// completed rhs is consumed at once by the Runge-Kutta combination of the 5 conserved cell fields,
+// out = c0*base + c1*(cur + dt*rhs) (O9), so rhs is neither written nor re-read and the update
+// traffic rides under the arithmetic of the sweep.  The old rhs / state values a cell needs are
+// loaded BEFORE the face arithmetic of the round, so their latency is hidden behind it.
+struct FluxUpd { const double *base[5]; const double *cur[5]; double *out[5]; double c0, c1; };
+
+template <int D, int NT, int MODE>
 __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
-                                             int want_amax) {
+                                             int want_amax, FluxUpd up) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
     constexpr int OD = 3 - D - TD;            // remaining axis
     constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
@@ -203,6 +224,8 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam
     const int nround = (nfr + R - 1) / R;
     const double mrh = -g.rh[D];
     double amax = 0.0;
+    const double dt = (MODE == 1) ? ctrl->dt : 0.0;
+    const int active = (MODE == 1) ? ctrl->active : 1;
 
     issue(0);
     issue(1);
@@ -211,23 +234,19 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam
         __syncthreads();
         if (t + 2 <= nround) issue(t + 2);
 
-        // (3) DER + divergence of the cells completed by round t-1
-        if (t >= 1) {
-            const int i = R * (t - 1) - 5 + a;            // cell row within the chunk
-            if (colok && i >= 0 && i < Cv) {
-                int sl[6];
-                int r0 = ((t - 1) % 3) * R - 5 + a;
-                if (r0 < 0) r0 += RL;
+        // (3a) cells completed by round t-1: issue the loads of what their update needs
+        const int i2 = R * (t - 1) - 5 + a;               // cell row within the chunk
+        const bool do2 = (t >= 1) && colok && i2 >= 0 && i2 < Cv;
+        const int o2 = ocol + sD * (m0 + i2);
+        double rold[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, ucur[5], ubase[5];
+        if (do2) {
+            if (D != 0) {
 #pragma unroll
-                for (int k = 0; k < 6; ++k) { sl[k] = r0 * FR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
-                const int o = ocol + sD * (m0 + i);
-                const double *Fb = sF + b * SB;
+                for (int c = 0; c < 5; ++c) rold[c] = __ldg(st.R[c] + o2);
+            }
+            if (MODE == 1) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) {
-                    const double *F = Fb + c * FV;
-                    const double r = mrh * der_diff(F[sl[0]], F[sl[1]], F[sl[2]], F[sl[3]], F[sl[4]], F[sl[5]]);
-                    if (D == 0) st.R[c][o] = r; else st.R[c][o] += r;
-                }
+                for (int c = 0; c < 5; ++c) { ucur[c] = __ldg(up.cur[c] + o2); ubase[c] = __ldg(up.base[c] + o2); }
             }
         }
 
@@ -262,6 +281,26 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam
                 st.vb[D][0][o] = vb1;
                 st.vb[D][1][o] = vb2;
                 amax = dmax(amax, dmax(ap, am));
+            }
+        }
+
+        // (3b) DER + divergence (O6) of the cells completed by round t-1
+        if (do2) {
+            int sl[6];
+            int r0 = ((t - 1) % 3) * R - 5 + a;
+            if (r0 < 0) r0 += RL;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) { sl[k] = r0 * FR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
+            const double *Fb = sF + b * SB;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                const double *F = Fb + c * FV;
+                const double r = rold[c] + mrh * der_diff(F[sl[0]], F[sl[1]], F[sl[2]], F[sl[3]], F[sl[4]], F[sl[5]]);
+                if (MODE == 1) {
+                    if (active) up.out[c][o2] = up.c0 * ubase[c] + up.c1 * (ucur[c] + dt * r);
+                } else {
+                    st.R[c][o2] = r;
+                }
             }
         }
     }
@@ -348,6 +387,7 @@ __device__ __forceinline__ double curl_comp(const Grid &g, const double *const E
              g.rh[K] * der_diff(b[0], b[1], b[2], b[3], b[4], b[5]));
 }
 
+template <bool WITH_U>
 __global__ void __launch_bounds__(256) k_update(Grid g, const double *E0, const double *E1, const double *E2,
                                                 const double *R0, const double *R1, const double *R2,
                                                 const double *R3, const double *R4, Update up, const Ctrl *ctrl,
@@ -368,13 +408,14 @@ __global__ void __launch_bounds__(256) k_update(Grid g, const double *E0, const 
         for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d]);
     }
     const double *const E[3] = {E0, E1, E2};
-    double r[8] = {__ldg(R0 + c), __ldg(R1 + c), __ldg(R2 + c), __ldg(R3 + c), __ldg(R4 + c), 0.0, 0.0, 0.0};
+    double r[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (WITH_U) { r[0] = __ldg(R0 + c); r[1] = __ldg(R1 + c); r[2] = __ldg(R2 + c); r[3] = __ldg(R3 + c); r[4] = __ldg(R4 + c); }
     r[5] = curl_comp<0>(g, E, ix);
     r[6] = curl_comp<1>(g, E, ix);
     r[7] = curl_comp<2>(g, E, ix);
     if (honour_active && !active) return;
 #pragma unroll
-    for (int v = 0; v < 8; ++v) {
+    for (int v = WITH_U ? 0 : 5; v < 8; ++v) {
         const double cur = up.cur[v][c];
         const double adv = cur + dt * r[v];
         up.out[v][c] = (up.c0 == 0.0) ? adv : up.c0 * up.base[v][c] + up.c1 * adv;
