@@ -153,7 +153,14 @@ int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePl
     if (want_amax == 2) {   // stage 1 of echo_step: dt must exist before any update (S9)
         KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
     }
-    KL(KC_UCT, "k_uct", k_uct<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st));
+    {   // plane-marching UCT: 16 x 8 tiles of (x, y), chunks of planes along z sized for >= ~8 blocks per SM
+        const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
+        int nchunk = (148 * 8 + tiles - 1) / tiles;
+        nchunk = std::max(1, std::min(nchunk, (g.n[2] + 15) / 16));
+        const int CZ = (g.n[2] + nchunk - 1) / nchunk;
+        dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
+        KL(KC_UCT, "k_uct2", k_uct2<<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
+    }
     return ECHO_OK;
 }
 

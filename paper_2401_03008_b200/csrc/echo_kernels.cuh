@@ -320,7 +320,12 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam
     }
 }
 
-// ------------------------------------------------------------------ point 4: UCT edge EMFs (O7)
+}  // namespace echo
+#include "echo_uct.cuh"   // k_uct2: the plane-marching UCT kernel used by echo_step
+namespace echo {
+
+// ------------------------------------------------------------------ point 4: UCT edge EMFs (O7) — reference form
+// (one thread per cell, every stencil through L1/L2; kept for grids whose x-y plane is tiny)
 // One thread per cell computes the three edge EMFs attached to it.  For the k-edge, with
 // i = (k+1)%3, j = (k+2)%3:   E_k = -HLL_i[ vbar_i B_j ] + HLL_j[ vbar_j B_i ]
 // where (vbar_i saved at j-faces, staggered B_j) are MP5-reconstructed along i and the edge speeds

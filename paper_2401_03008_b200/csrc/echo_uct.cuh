@@ -1,0 +1,181 @@
+// echo_uct.cuh — point 4 of a sub-step: the UCT edge EMFs (O7), plane-marching version.
+//
+// A block owns a TX x TY = 16 x 8 tile of (x, y) and marches along z over a chunk of planes, one
+// plane per round, one cell (three edges) per thread.  What a plane needs:
+//   XR  4 fields reconstructed along x  (vbar_x@y-face, B_y, vbar_x@z-face, B_z): (TX+5) x TY
+//   YR  4 fields reconstructed along y  (vbar_y@x-face, B_x, vbar_y@z-face, B_z): TX x (TY+5)
+//   ZW  4 fields reconstructed along z  (vbar_z@x-face, B_x, vbar_z@y-face, B_y): a 6-plane sliding
+//       window per thread, held in REGISTERS (one new value per field and plane)
+//   AX, AY, AZ  the saved a+/a- of the three directions at the cell and its +1 neighbours along the
+//       two other axes (the edge speed is the max over the two faces adjacent to the edge)
+// XR/YR/AZ of plane k+1 and AX/AY of plane k+2 are brought in by cp.async (LDGSTS) while plane k is
+// computed (double / triple buffers), with the periodic wrap applied to the source coordinates, so
+// every input is read from L2/HBM about once (plus tile halos) and the global-memory latency hides
+// behind the arithmetic.  One __syncthreads per plane.
+#pragma once
+#include "echo_math.cuh"
+#include "echo_types.cuh"
+
+namespace echo {
+
+constexpr int UCT_TX = 16, UCT_TY = 8, UCT_NT = UCT_TX * UCT_TY;
+constexpr int UCT_XRW = UCT_TX + 5, UCT_XR = UCT_XRW * UCT_TY;          // 21 x 8
+constexpr int UCT_YRH = UCT_TY + 5, UCT_YR = UCT_TX * UCT_YRH;          // 16 x 13
+constexpr int UCT_AX = UCT_TX * (UCT_TY + 1);                           // 16 x 9   (c, c+e_y)
+constexpr int UCT_AYW = UCT_TX + 1, UCT_AY = UCT_AYW * UCT_TY;          // 17 x 8   (c, c+e_x)
+constexpr int UCT_AZ = UCT_AYW * (UCT_TY + 1);                          // 17 x 9   (c, c+e_x, c+e_y)
+
+// HLL-upwinded product of O7: [a+ vL BL + a- vR BR - a+ a- (BR - BL)] / (a+ + a-)
+__device__ __forceinline__ double uct_hll(double ap, double am, double vL, double vR, double BL, double BR) {
+    return (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) * rcp_fast(ap + am);
+}
+
+__global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
+    __shared__ double sXR[2][4][UCT_XR];
+    __shared__ double sYR[2][4][UCT_YR];
+    __shared__ double sAZ[2][2][UCT_AZ];
+    __shared__ double sAX[3][2][UCT_AX];
+    __shared__ double sAY[3][2][UCT_AY];
+
+    const int tid = threadIdx.x;
+    const int tx = tid % UCT_TX, ty = tid / UCT_TX;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int x0 = blockIdx.x * UCT_TX, y0 = blockIdx.y * UCT_TY, z0 = blockIdx.z * CZ;
+    const int CZv = min(CZ, nz - z0);
+    const int sy = g.s[1], sz = g.s[2];
+
+    // in-plane source offsets of the (at most two) elements this thread copies per region
+    int oXR[2], oYR[2], oAX[2], oAY[2], oAZ[2];
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int e = tid + UCT_NT * it;
+        oXR[it] = (e < UCT_XR) ? wrapi(x0 - 2 + e % UCT_XRW, nx) + sy * wrapi(y0 + e / UCT_XRW, ny) : -1;
+        oYR[it] = (e < UCT_YR) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 - 2 + e / UCT_TX, ny) : -1;
+        oAX[it] = (e < UCT_AX) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 + e / UCT_TX, ny) : -1;
+        oAY[it] = (e < UCT_AY) ? wrapi(x0 + e % UCT_AYW, nx) + sy * wrapi(y0 + e / UCT_AYW, ny) : -1;
+        oAZ[it] = (e < UCT_AZ) ? wrapi(x0 + e % UCT_AYW, nx) + sy * wrapi(y0 + e / UCT_AYW, ny) : -1;
+    }
+    // XR = {vbar_x@y, B_y, vbar_x@z, B_z}; YR = {vbar_y@x, B_x, vbar_y@z, B_z}; ZW = {vbar_z@x, B_x, vbar_z@y, B_y}
+    // (direction d saves vbar_{(d+1)%3} in slot 0 and vbar_{(d+2)%3} in slot 1)
+    const double *fXR[4] = {st.vb[1][1], st.Bf[1], st.vb[2][0], st.Bf[2]};
+    const double *fYR[4] = {st.vb[0][0], st.Bf[0], st.vb[2][1], st.Bf[2]};
+    const double *fZW[4] = {st.vb[0][1], st.Bf[0], st.vb[1][0], st.Bf[1]};
+
+    auto issue_plane = [&](int k, int slot) {          // XR, YR, AZ of plane k
+        const int pz = sz * wrapi(k, nz);
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = tid + UCT_NT * it;
+            if (oXR[it] >= 0) {
+#pragma unroll
+                for (int f = 0; f < 4; ++f) cp_async8(&sXR[slot][f][e], fXR[f] + (pz + oXR[it]));
+            }
+            if (oYR[it] >= 0) {
+#pragma unroll
+                for (int f = 0; f < 4; ++f) cp_async8(&sYR[slot][f][e], fYR[f] + (pz + oYR[it]));
+            }
+            if (oAZ[it] >= 0) {
+                cp_async8(&sAZ[slot][0][e], st.ap[2] + (pz + oAZ[it]));
+                cp_async8(&sAZ[slot][1][e], st.am[2] + (pz + oAZ[it]));
+            }
+        }
+    };
+    auto issue_speeds = [&](int k, int slot) {         // AX, AY of plane k
+        const int pz = sz * wrapi(k, nz);
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = tid + UCT_NT * it;
+            if (oAX[it] >= 0) {
+                cp_async8(&sAX[slot][0][e], st.ap[0] + (pz + oAX[it]));
+                cp_async8(&sAX[slot][1][e], st.am[0] + (pz + oAX[it]));
+            }
+            if (oAY[it] >= 0) {
+                cp_async8(&sAY[slot][0][e], st.ap[1] + (pz + oAY[it]));
+                cp_async8(&sAY[slot][1][e], st.am[1] + (pz + oAY[it]));
+            }
+        }
+    };
+
+    // this thread's cell column (clamped for the loads of ragged tiles; stores are masked)
+    const bool cellok = (x0 + tx < nx) && (y0 + ty < ny);
+    const int ccol = min(x0 + tx, nx - 1) + sy * min(y0 + ty, ny - 1);
+
+    // prologue: plane z0 (+ speeds of z0 and z0+1) by cp.async; z-window planes z0-2 .. z0+3 directly
+    issue_plane(z0, 0);
+    issue_speeds(z0, 0);
+    issue_speeds(z0 + 1, 1);
+    cp_async_commit();
+    double zw[4][6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+        const int pz = sz * wrapi(z0 - 2 + m, nz);
+#pragma unroll
+        for (int f = 0; f < 4; ++f) zw[f][m] = __ldg(fZW[f] + (pz + ccol));
+    }
+
+    for (int r = 0; r < CZv; ++r) {
+        const int k = z0 + r;
+        cp_async_wait_all();
+        __syncthreads();
+        const bool more = (r + 1 < CZv);
+        double znew[4] = {0.0, 0.0, 0.0, 0.0};
+        if (more) {
+            issue_plane(k + 1, (r + 1) & 1);
+            issue_speeds(k + 2, (r + 2) % 3);
+            cp_async_commit();
+            const int pz = sz * wrapi(k + 4, nz);
+#pragma unroll
+            for (int f = 0; f < 4; ++f) znew[f] = __ldg(fZW[f] + (pz + ccol));
+        }
+
+        if (cellok) {
+            const int ps = r & 1, as0 = r % 3, as1 = (r + 1) % 3;
+            // MP5 L/R at the edge for the 4 x-, 4 y- and 4 z-reconstructed fields
+            double xL[4], xR[4], yL[4], yR[4], zL[4], zR[4];
+#pragma unroll
+            for (int f = 0; f < 4; ++f) {
+                const double *p = &sXR[ps][f][ty * UCT_XRW + tx];
+                xL[f] = mp5(p[0], p[1], p[2], p[3], p[4]);
+                xR[f] = mp5(p[5], p[4], p[3], p[2], p[1]);
+                const double *q = &sYR[ps][f][ty * UCT_TX + tx];
+                yL[f] = mp5(q[0], q[UCT_TX], q[2 * UCT_TX], q[3 * UCT_TX], q[4 * UCT_TX]);
+                yR[f] = mp5(q[5 * UCT_TX], q[4 * UCT_TX], q[3 * UCT_TX], q[2 * UCT_TX], q[UCT_TX]);
+                zL[f] = mp5(zw[f][0], zw[f][1], zw[f][2], zw[f][3], zw[f][4]);
+                zR[f] = mp5(zw[f][5], zw[f][4], zw[f][3], zw[f][2], zw[f][1]);
+            }
+            // saved speeds at the cell and its +1 neighbours
+            const int iax = ty * UCT_TX + tx, iay = ty * UCT_AYW + tx;
+            const double axp = sAX[as0][0][iax], axm = sAX[as0][1][iax];
+            const double ayp = sAY[as0][0][iay], aym = sAY[as0][1][iay];
+            const double azp = sAZ[ps][0][iay], azm = sAZ[ps][1][iay];
+            // E_z: i = x, j = y
+            const double ez = -uct_hll(dmax(axp, sAX[as0][0][iax + UCT_TX]), dmax(axm, sAX[as0][1][iax + UCT_TX]),
+                                       xL[0], xR[0], xL[1], xR[1]) +
+                              uct_hll(dmax(ayp, sAY[as0][0][iay + 1]), dmax(aym, sAY[as0][1][iay + 1]),
+                                      yL[0], yR[0], yL[1], yR[1]);
+            // E_y: i = z, j = x
+            const double ey = -uct_hll(dmax(azp, sAZ[ps][0][iay + 1]), dmax(azm, sAZ[ps][1][iay + 1]),
+                                       zL[0], zR[0], zL[1], zR[1]) +
+                              uct_hll(dmax(axp, sAX[as1][0][iax]), dmax(axm, sAX[as1][1][iax]),
+                                      xL[2], xR[2], xL[3], xR[3]);
+            // E_x: i = y, j = z
+            const double ex = -uct_hll(dmax(ayp, sAY[as1][0][iay]), dmax(aym, sAY[as1][1][iay]),
+                                       yL[2], yR[2], yL[3], yR[3]) +
+                              uct_hll(dmax(azp, sAZ[ps][0][iay + UCT_AYW]), dmax(azm, sAZ[ps][1][iay + UCT_AYW]),
+                                      zL[2], zR[2], zL[3], zR[3]);
+            const int o = sz * k + ccol;
+            st.E[0][o] = ex;
+            st.E[1][o] = ey;
+            st.E[2][o] = ez;
+        }
+        // slide the z-window
+#pragma unroll
+        for (int f = 0; f < 4; ++f) {
+#pragma unroll
+            for (int m = 0; m < 5; ++m) zw[f][m] = zw[f][m + 1];
+            zw[f][5] = znew[f];
+        }
+    }
+}
+
+}  // namespace echo
