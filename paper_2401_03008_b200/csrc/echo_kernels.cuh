@@ -265,8 +265,7 @@ __global__ void __launch_bounds__(NT) k_flux(Grid g, Stage st, int C, double gam
             for (int v = 0; v < 7; ++v) {
                 const double *p = Pb + v * SV;
                 const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
-                qL[slot[v]] = mp5(s0, s1, s2, s3, s4);
-                qR[slot[v]] = mp5(s5, s4, s3, s2, s1);
+                mp5_pair<true>(s0, s1, s2, s3, s4, s5, qL[slot[v]], qR[slot[v]]);
             }
             qL[5 + D] = qR[5 + D] = Pb[7 * SV + sl[2]];   // the normal B is the staggered value
             double F[5], ap, am, vb1, vb2;

@@ -95,16 +95,57 @@ __device__ __forceinline__ double mp5_limit(double vm2, double vm1, double v0, d
     const double vmax = dmin(mx1, mx2);
     return vor + minmod2(vmin - vor, vmax - vor);
 }
+__device__ __noinline__ double mp5_limit_call(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
+    return mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
+}
+// INL: limiter inlined behind a branch (flux sweeps) or called out of line (UCT kernel, whose 24
+// reconstructions would otherwise overflow the instruction cache).
+template <bool INL = true>
 __device__ __forceinline__ double mp5(double vm2, double vm1, double v0, double vp1, double vp2) {
     const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
                        ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
     const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
     double r = vor;
     if ((vor - v0) * (vor - vmp) > 1e-10) {
-        asm volatile("" ::: "memory");   // keeps this a real branch: the limiter must not be if-converted
-        r = mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
+        if (INL) {
+            asm volatile("" ::: "memory");   // keeps this a real branch: the limiter must not be if-converted
+            r = mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
+        } else {
+            r = mp5_limit_call(vm2, vm1, v0, vp1, vp2, vor);
+        }
     }
     return r;
+}
+
+// Both one-sided values at the face between s2 and s3 from the six cells s0..s5 around it:
+// L = MP5(s0..s4) centred on s2, R = MP5(s5..s1) centred on s3 (mirrored).  The S&H test is evaluated
+// as t (t - mm) > eps with t = vOR - v_i and mm = minmod(v_{i+1} - v_i, 4 (v_i - v_{i-1})): the two sides
+// share s3 - s2, and the factor 4 is an exact exponent bump on the integer pipe (a zero becomes
+// 2^-1021, which minmod treats like the zero it stands for).
+__device__ __forceinline__ double times4(double d) {
+    return __hiloint2double(__double2hiint(d) + 0x00200000, __double2loint(d));
+}
+template <bool INL = true>
+__device__ __forceinline__ void mp5_pair(double s0, double s1, double s2, double s3, double s4, double s5, double &L,
+                                         double &R) {
+    const double vorL = (3.0 / 128.0) * s0 + ((-20.0 / 128.0) * s1 + ((90.0 / 128.0) * s2 +
+                        ((60.0 / 128.0) * s3 + (-5.0 / 128.0) * s4)));
+    const double vorR = (3.0 / 128.0) * s5 + ((-20.0 / 128.0) * s4 + ((90.0 / 128.0) * s3 +
+                        ((60.0 / 128.0) * s2 + (-5.0 / 128.0) * s1)));
+    const double d23 = s3 - s2;
+    const double mmL = minmod2(d23, times4(s2 - s1));
+    const double mmR = minmod2(-d23, times4(s3 - s4));
+    const double tL = vorL - s2, tR = vorR - s3;
+    L = vorL;
+    R = vorR;
+    if (tL * (tL - mmL) > 1e-10) {
+        if (INL) { asm volatile("" ::: "memory"); L = mp5_limit(s0, s1, s2, s3, s4, vorL); }
+        else L = mp5_limit_call(s0, s1, s2, s3, s4, vorL);
+    }
+    if (tR * (tR - mmR) > 1e-10) {
+        if (INL) { asm volatile("" ::: "memory"); R = mp5_limit(s5, s4, s3, s2, s1, vorR); }
+        else R = mp5_limit_call(s5, s4, s3, s2, s1, vorR);
+    }
 }
 
 // ---------------------------------------------------------------- point physics
@@ -125,6 +166,9 @@ __device__ __forceinline__ void prim2cons(double gg, const double q[8], double u
 }
 
 // One side of a D-face: conserved state u, physical flux f (eq.(8)), fast speeds lp, lm (O4).
+// With E = -v x B:  E^2 = B^2 - b2,  b2 = B^2 (1 - v^2) + (v.B)^2,  S = (y + B^2) v - (v.B) B, and
+//   F_D(S_a) = S_a v_D - B_D beta_a + delta_aD (p + b2/2),  beta_a = (1 - v^2) B_a + (v.B) v_a,
+// which is eq.(8)'s  y v_a v_D - E_a E_D - B_a B_D + p_tot delta_aD  after expanding (v x B)_a (v x B)_D.
 template <int D>
 __device__ __forceinline__ void side_state(double gam, double gg, const double q[8], double u[5], double f[5],
                                            double &lp, double &lm) {
@@ -139,22 +183,19 @@ __device__ __forceinline__ void side_state(double gam, double gg, const double q
     const double rhoh = rho + gg * p;
     const double y = rhoh * (W * W);
     const double yb = y + B2;
-    const double E2 = v2 * B2 - vB * vB;
-    const double ptot = p + 0.5 * (E2 + B2);
-    // E = -v x B
-    const double E[3] = {-(v[1] * B[2] - v[2] * B[1]), -(v[2] * B[0] - v[0] * B[2]), -(v[0] * B[1] - v[1] * B[0])};
+    const double b2 = fma(B2, omv2, vB * vB);
     u[0] = rho * W;
-    u[1] = yb * v[0] - vB * B[0];
-    u[2] = yb * v[1] - vB * B[1];
-    u[3] = yb * v[2] - vB * B[2];
-    u[4] = y - p + 0.5 * (E2 + B2);
-    const double yvd = y * v[D];
+    u[4] = fma(-0.5, b2, (y - p) + B2);
     f[0] = u[0] * v[D];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) f[1 + a] = yvd * v[a] - E[a] * E[D] - B[a] * B[D] + (a == D ? ptot : 0.0);
+    for (int a = 0; a < 3; ++a) {
+        u[1 + a] = yb * v[a] - vB * B[a];
+        const double beta = fma(omv2, B[a], vB * v[a]);
+        f[1 + a] = fma(u[1 + a], v[D], -(B[D] * beta));
+    }
+    f[1 + D] += fma(0.5, b2, p);
     f[4] = u[1 + D];
     // O4: a^2 = cs^2 + ca^2 - cs^2 ca^2, cs^2 = gamma p/(rho h), ca^2 = b^2/(rho h + b^2)
-    const double b2 = B2 * omv2 + vB * vB;
     const double w = rhoh + b2;
     const double r = rcp_fast(rhoh * w);
     const double cs2 = gam * p * w * r;

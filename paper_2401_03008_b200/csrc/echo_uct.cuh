@@ -130,39 +130,43 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
 
         if (cellok) {
             const int ps = r & 1, as0 = r % 3, as1 = (r + 1) % 3;
-            // MP5 L/R at the edge for the 4 x-, 4 y- and 4 z-reconstructed fields
-            double xL[4], xR[4], yL[4], yR[4], zL[4], zR[4];
-#pragma unroll
-            for (int f = 0; f < 4; ++f) {
-                const double *p = &sXR[ps][f][ty * UCT_XRW + tx];
-                xL[f] = mp5(p[0], p[1], p[2], p[3], p[4]);
-                xR[f] = mp5(p[5], p[4], p[3], p[2], p[1]);
-                const double *q = &sYR[ps][f][ty * UCT_TX + tx];
-                yL[f] = mp5(q[0], q[UCT_TX], q[2 * UCT_TX], q[3 * UCT_TX], q[4 * UCT_TX]);
-                yR[f] = mp5(q[5 * UCT_TX], q[4 * UCT_TX], q[3 * UCT_TX], q[2 * UCT_TX], q[UCT_TX]);
-                zL[f] = mp5(zw[f][0], zw[f][1], zw[f][2], zw[f][3], zw[f][4]);
-                zR[f] = mp5(zw[f][5], zw[f][4], zw[f][3], zw[f][2], zw[f][1]);
-            }
             // saved speeds at the cell and its +1 neighbours
             const int iax = ty * UCT_TX + tx, iay = ty * UCT_AYW + tx;
             const double axp = sAX[as0][0][iax], axm = sAX[as0][1][iax];
             const double ayp = sAY[as0][0][iay], aym = sAY[as0][1][iay];
             const double azp = sAZ[ps][0][iay], azm = sAZ[ps][1][iay];
+            // one upwinded product at a time: MP5 L/R (O3) of (vbar, B) to the edge, then O7
+            auto along_x = [&](int f, double ap, double am) {
+                const double *p = &sXR[ps][f][ty * UCT_XRW + tx], *q = p + UCT_XR;
+                double vL, vR, BL, BR;
+                mp5_pair<false>(p[0], p[1], p[2], p[3], p[4], p[5], vL, vR);
+                mp5_pair<false>(q[0], q[1], q[2], q[3], q[4], q[5], BL, BR);
+                return uct_hll(ap, am, vL, vR, BL, BR);
+            };
+            auto along_y = [&](int f, double ap, double am) {
+                const double *p = &sYR[ps][f][ty * UCT_TX + tx], *q = p + UCT_YR;
+                constexpr int S = UCT_TX;
+                double vL, vR, BL, BR;
+                mp5_pair<false>(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+                mp5_pair<false>(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+                return uct_hll(ap, am, vL, vR, BL, BR);
+            };
+            auto along_z = [&](int f, double ap, double am) {
+                const double *p = zw[f], *q = zw[f + 1];
+                double vL, vR, BL, BR;
+                mp5_pair<false>(p[0], p[1], p[2], p[3], p[4], p[5], vL, vR);
+                mp5_pair<false>(q[0], q[1], q[2], q[3], q[4], q[5], BL, BR);
+                return uct_hll(ap, am, vL, vR, BL, BR);
+            };
             // E_z: i = x, j = y
-            const double ez = -uct_hll(dmax(axp, sAX[as0][0][iax + UCT_TX]), dmax(axm, sAX[as0][1][iax + UCT_TX]),
-                                       xL[0], xR[0], xL[1], xR[1]) +
-                              uct_hll(dmax(ayp, sAY[as0][0][iay + 1]), dmax(aym, sAY[as0][1][iay + 1]),
-                                      yL[0], yR[0], yL[1], yR[1]);
+            const double ez = -along_x(0, dmax(axp, sAX[as0][0][iax + UCT_TX]), dmax(axm, sAX[as0][1][iax + UCT_TX])) +
+                              along_y(0, dmax(ayp, sAY[as0][0][iay + 1]), dmax(aym, sAY[as0][1][iay + 1]));
             // E_y: i = z, j = x
-            const double ey = -uct_hll(dmax(azp, sAZ[ps][0][iay + 1]), dmax(azm, sAZ[ps][1][iay + 1]),
-                                       zL[0], zR[0], zL[1], zR[1]) +
-                              uct_hll(dmax(axp, sAX[as1][0][iax]), dmax(axm, sAX[as1][1][iax]),
-                                      xL[2], xR[2], xL[3], xR[3]);
+            const double ey = -along_z(0, dmax(azp, sAZ[ps][0][iay + 1]), dmax(azm, sAZ[ps][1][iay + 1])) +
+                              along_x(2, dmax(axp, sAX[as1][0][iax]), dmax(axm, sAX[as1][1][iax]));
             // E_x: i = y, j = z
-            const double ex = -uct_hll(dmax(ayp, sAY[as1][0][iay]), dmax(aym, sAY[as1][1][iay]),
-                                       yL[2], yR[2], yL[3], yR[3]) +
-                              uct_hll(dmax(azp, sAZ[ps][0][iay + UCT_AYW]), dmax(azm, sAZ[ps][1][iay + UCT_AYW]),
-                                      zL[2], zR[2], zL[3], zR[3]);
+            const double ex = -along_y(2, dmax(ayp, sAY[as1][0][iay]), dmax(aym, sAY[as1][1][iay])) +
+                              along_z(2, dmax(azp, sAZ[ps][0][iay + UCT_AYW]), dmax(azm, sAZ[ps][1][iay + UCT_AYW]));
             const int o = sz * k + ccol;
             st.E[0][o] = ex;
             st.E[1][o] = ey;
