@@ -175,12 +175,17 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
     up.c0 = c0;
     up.c1 = c1;
     const Grid &g = ctx->g;
-    if (with_u)
+    if (with_u) {
         KL(KC_UPDATE, "k_update", k_update<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1],
                                                                               st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
-    else
-        KL(KC_UPDATE, "k_update", k_update<false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1],
-                                                                               st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
+    } else {   // staggered B only: plane-marching curl + update
+        const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
+        int nchunk = (148 * 16 + tiles - 1) / tiles;
+        nchunk = std::max(1, std::min(nchunk, (g.n[2] + 15) / 16));
+        const int CZ = (g.n[2] + nchunk - 1) / nchunk;
+        dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
+        KL(KC_UPDATE, "k_bupd", k_bupd<<<grid, UCT_NT, 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], up, ctx->ctrl, CZ));
+    }
     return ECHO_OK;
 }
 

@@ -183,3 +183,116 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
 }
 
 }  // namespace echo
+
+// ------------------------------------------------------------------ points 4b + 5 for the staggered B
+// k_bupd: curl of the DER-corrected edge EMFs (O8, eq.(10)) and the Runge-Kutta combination of the
+// three face fields (O9), plane-marching like k_uct2: the x- and y-stencils of a plane come from
+// cp.async-fed tiles (one plane ahead), the z-stencils from a 6-plane register window, the old B values
+// of the next plane are loaded one round early.  Pure streaming: 12 doubles per cell.
+//   dB_x/dt = -[D_y E_z - D_z E_y],  dB_y/dt = -[D_z E_x - D_x E_z],  dB_z/dt = -[D_x E_y - D_y E_x]
+// with D_d the 6-point DER+difference stencil over cells c-3 .. c+2 along d.
+namespace echo {
+
+constexpr int BU_XE = UCT_XRW * UCT_TY;     // 21 x 8, x offsets -3 .. TX+1
+constexpr int BU_YE = UCT_TX * UCT_YRH;     // 16 x 13, y offsets -3 .. TY+1
+
+__global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const double *E1, const double *E2, Update up,
+                                                 const Ctrl *ctrl, int CZ) {
+    __shared__ double sXE[2][2][BU_XE];    // fields: E_z, E_y (differenced along x)
+    __shared__ double sYE[2][2][BU_YE];    // fields: E_z, E_x (differenced along y)
+    const int tid = threadIdx.x;
+    const int tx = tid % UCT_TX, ty = tid / UCT_TX;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int x0 = blockIdx.x * UCT_TX, y0 = blockIdx.y * UCT_TY, z0 = blockIdx.z * CZ;
+    const int CZv = min(CZ, nz - z0);
+    const int sy = g.s[1], sz = g.s[2];
+    const double dt = ctrl->dt;
+    const int active = ctrl->active;
+
+    int oXE[2], oYE[2];
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int e = tid + UCT_NT * it;
+        oXE[it] = (e < BU_XE) ? wrapi(x0 - 3 + e % UCT_XRW, nx) + sy * wrapi(y0 + e / UCT_XRW, ny) : -1;
+        oYE[it] = (e < BU_YE) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 - 3 + e / UCT_TX, ny) : -1;
+    }
+    auto issue_plane = [&](int k, int slot) {
+        const int pz = sz * wrapi(k, nz);
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = tid + UCT_NT * it;
+            if (oXE[it] >= 0) {
+                cp_async8(&sXE[slot][0][e], E2 + (pz + oXE[it]));
+                cp_async8(&sXE[slot][1][e], E1 + (pz + oXE[it]));
+            }
+            if (oYE[it] >= 0) {
+                cp_async8(&sYE[slot][0][e], E2 + (pz + oYE[it]));
+                cp_async8(&sYE[slot][1][e], E0 + (pz + oYE[it]));
+            }
+        }
+        cp_async_commit();
+    };
+    const bool cellok = (x0 + tx < nx) && (y0 + ty < ny);
+    const int ccol = min(x0 + tx, nx - 1) + sy * min(y0 + ty, ny - 1);
+
+    issue_plane(z0, 0);
+    double wy[6], wx[6];                   // z-windows of E_y and E_x: planes k-3 .. k+2
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+        const int pz = sz * wrapi(z0 - 3 + m, nz);
+        wy[m] = __ldg(E1 + (pz + ccol));
+        wx[m] = __ldg(E0 + (pz + ccol));
+    }
+    double bc[3], bb[3];                   // cur and base B of the plane about to be updated
+    {
+        const int o = sz * z0 + ccol;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { bc[d] = up.cur[5 + d][o]; bb[d] = __ldg(up.base[5 + d] + o); }
+    }
+
+    for (int r = 0; r < CZv; ++r) {
+        const int k = z0 + r;
+        cp_async_wait_all();
+        __syncthreads();
+        const bool more = (r + 1 < CZv);
+        double nwy = 0.0, nwx = 0.0, nbc[3] = {0.0, 0.0, 0.0}, nbb[3] = {0.0, 0.0, 0.0};
+        if (more) {
+            issue_plane(k + 1, (r + 1) & 1);
+            const int pz = sz * wrapi(k + 3, nz);
+            nwy = __ldg(E1 + (pz + ccol));
+            nwx = __ldg(E0 + (pz + ccol));
+            const int o = sz * (k + 1) + ccol;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { nbc[d] = up.cur[5 + d][o]; nbb[d] = __ldg(up.base[5 + d] + o); }
+        }
+        if (cellok && active) {
+            const int ps = r & 1;
+            const double *pz_x = &sXE[ps][0][ty * UCT_XRW + tx], *py_x = pz_x + BU_XE;     // E_z, E_y along x
+            const double *pz_y = &sYE[ps][0][ty * UCT_TX + tx], *px_y = pz_y + BU_YE;      // E_z, E_x along y
+            constexpr int S = UCT_TX;
+            const double dxEz = der_diff(pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
+            const double dxEy = der_diff(py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
+            const double dyEz = der_diff(pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
+            const double dyEx = der_diff(px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
+            const double dzEy = der_diff(wy[0], wy[1], wy[2], wy[3], wy[4], wy[5]);
+            const double dzEx = der_diff(wx[0], wx[1], wx[2], wx[3], wx[4], wx[5]);
+            double rb[3];
+            rb[0] = -(g.rh[1] * dyEz - g.rh[2] * dzEy);
+            rb[1] = -(g.rh[2] * dzEx - g.rh[0] * dxEz);
+            rb[2] = -(g.rh[0] * dxEy - g.rh[1] * dyEx);
+            const int o = sz * k + ccol;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const double adv = bc[d] + dt * rb[d];
+                up.out[5 + d][o] = (up.c0 == 0.0) ? adv : up.c0 * bb[d] + up.c1 * adv;
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < 5; ++m) { wy[m] = wy[m + 1]; wx[m] = wx[m + 1]; }
+        wy[5] = nwy; wx[5] = nwx;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { bc[d] = nbc[d]; bb[d] = nbb[d]; }
+    }
+}
+
+}  // namespace echo
