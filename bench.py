@@ -25,17 +25,22 @@ GAMMA, CFL = 4.0 / 3.0, 0.3
 SETK = "rho vx vy vz p bxf byf bzf".split()
 
 # Algorithmic work per cell and per launch.
-# flop: nominal FP64 operation count of the scheme; dbl: FP64 words read+written once per cell.
+# flop: nominal FP64 operation count of the scheme; dbl: FP64 words read+written once per cell by the
+# kernel as built, averaged over the three RK stages where the stages differ:
+#   k_prim   5 U + 3 B in, 5 prims + 3 centred B out = 16; stage 2 also reads rhs (5) and writes U1 (5)
+#   k_flux_x 8 in, 5 rhs + 4 saved face fields out = 17;  k_flux_y the same + 5 rhs in = 22
+#   k_flux_z stage 1: 22; stages 2-3 (RK combination fused): + U cur (5) + U^n (5) in, U out instead of rhs = 32
+#   k_uct    6 speeds + 6 vbar + 3 B in, 3 E out = 18;  k_update (staggered B): 3 E + 3 + 3 in, 3 out (stage 1: 9)
 ALGO = {
-    "k_prim":   {"flop": 24 + 268, "dbl": 16},
+    "k_prim":   {"flop": 24 + 268, "dbl": (16 + 26 + 16) / 3.0},
     "k_flux_x": {"flop": 614, "dbl": 17},
     "k_flux_y": {"flop": 614, "dbl": 22},
-    "k_flux_z": {"flop": 614, "dbl": 22},
+    "k_flux_z": {"flop": 614 + 32 * 2 / 3.0, "dbl": (22 + 32 + 32) / 3.0},
     "k_uct":    {"flop": 3 * 194, "dbl": 18},
-    "k_update": {"flop": 60 + 32, "dbl": (24 + 32 + 32) / 3.0},
+    "k_update": {"flop": 60 + 12, "dbl": (9 + 12 + 12) / 3.0},
 }
-FLOP_PER_CELL_UPDATE = 3 * sum(v["flop"] for v in ALGO.values())          # 8424
-BYTES_PER_CELL_UPDATE = 8 * 3 * sum(v["dbl"] for v in ALGO.values())      # 2984
+FLOP_PER_CELL_UPDATE = 3 * sum(v["flop"] for v in ALGO.values())          # ~8.4e3
+BYTES_PER_CELL_UPDATE = 8 * 3 * sum(v["dbl"] for v in ALGO.values())      # 2784
 
 
 def measured_peaks():
@@ -98,6 +103,23 @@ class ClockSampler:
             out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), samples=len(sm))
         out["reasons"] = sorted(reasons)
         return out
+
+
+def max_over_ranks(value, device, world):
+    """Max over ranks of a host float (NCCL on the GPU, gloo in the CPU tests); identity for one rank."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(cells_per_rank, steps, ms_local, device, world):
+    """Whole-job cell-updates/s: all ranks' cells x steps / the slowest rank's device time."""
+    ms = max_over_ranks(ms_local, device, world)
+    return world * cells_per_rank * steps / (ms * 1e-3), ms
 
 
 def oracle_rate(n, steps, warmup=0, direction="diag"):
@@ -165,11 +187,11 @@ def run_gpu(args):
         torch.cuda.synchronize()
 
     # ---- device-resident throughput: W warm-up steps, then EXACTLY K timed steps
+    sampler = ClockSampler(local)       # started before the warm-up so that nvidia-smi is already polling
+    sampler.start()                     # when the timed region begins (samples cover warm-up + timed steps)
     e.step(W)
     barrier()
     e.timing(True)                      # per-kernel CUDA-event brackets on the launching stream
-    sampler = ClockSampler(local)
-    sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
@@ -182,11 +204,7 @@ def run_gpu(args):
     e.timing(False)
     d = e.diagnostics()
     assert d["rc"] == 0 and d["steps"] == W + K, d
-    tt = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_max = float(tt.item())
-    value = world * N * K / (ms_max * 1e-3)
+    value, ms_max = whole_job_rate(N, K, ms, "cuda", world)
 
     # ---- end to end through the C ABI with HOST buffers: every step uploads its inputs from pinned host
     # memory (echo_set_primitives_host), advances one RK3 step and reads the primitives back to the host
@@ -202,10 +220,7 @@ def run_gpu(args):
         e.get_primitives_host(outs)
     ev1.record()
     barrier()
-    te = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * N * Ke / (float(te.item()) * 1e-3)
+    e2e_value, _ = whole_job_rate(N, Ke, ev0.elapsed_time(ev1), "cuda", world)
     # sanity of what came back: one step of the wave stays within truncation error of the input
     assert abs(float(outs[0].mean()) - 1.0) < 1e-6
 

@@ -177,7 +177,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 struct FluxUpd { const double *base[5]; const double *cur[5]; double *out[5]; double c0, c1; };
 
 template <int D, int NT, int MODE>
-__global__ void __launch_bounds__(NT, MODE == 0 ? 5 : 4) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
+__global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
                                              int want_amax, FluxUpd up) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
     constexpr int OD = 3 - D - TD;            // remaining axis
