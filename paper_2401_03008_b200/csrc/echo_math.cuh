@@ -148,6 +148,25 @@ __device__ __forceinline__ void mp5_pair(double s0, double s1, double s2, double
     }
 }
 
+// Branch-free first half of mp5_pair: the two unlimited values and the two S&H test bits (bit 0: L needs the
+// limiter, bit 1: R); mp5_pair_fix applies the limiter afterwards.  Used where several stencils should be
+// interleaved by the compiler before any branch (k_uct2).
+__device__ __forceinline__ unsigned mp5_pair_fast(double s0, double s1, double s2, double s3, double s4, double s5,
+                                                  double &L, double &R) {
+    L = (3.0 / 128.0) * s0 + ((-20.0 / 128.0) * s1 + ((90.0 / 128.0) * s2 + ((60.0 / 128.0) * s3 + (-5.0 / 128.0) * s4)));
+    R = (3.0 / 128.0) * s5 + ((-20.0 / 128.0) * s4 + ((90.0 / 128.0) * s3 + ((60.0 / 128.0) * s2 + (-5.0 / 128.0) * s1)));
+    const double d23 = s3 - s2;
+    const double mmL = minmod2(d23, times4(s2 - s1));
+    const double mmR = minmod2(-d23, times4(s3 - s4));
+    const double tL = L - s2, tR = R - s3;
+    return (tL * (tL - mmL) > 1e-10 ? 1u : 0u) | (tR * (tR - mmR) > 1e-10 ? 2u : 0u);
+}
+__device__ __forceinline__ void mp5_pair_fix(unsigned bits, double s0, double s1, double s2, double s3, double s4,
+                                             double s5, double &L, double &R) {
+    if (bits & 1u) L = mp5_limit_call(s0, s1, s2, s3, s4, L);
+    if (bits & 2u) R = mp5_limit_call(s5, s4, s3, s2, s1, R);
+}
+
 // ---------------------------------------------------------------- point physics
 // q[8] = (rho, vx, vy, vz, p, Bx, By, Bz); u[5] = (D, Sx, Sy, Sz, U).  gg = gamma/(gamma-1).
 // Identities used (E = -v x B): E x B = B^2 v - (v.B) B, E^2 = v^2 B^2 - (v.B)^2.

@@ -136,28 +136,25 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
             const double ayp = sAY[as0][0][iay], aym = sAY[as0][1][iay];
             const double azp = sAZ[ps][0][iay], azm = sAZ[ps][1][iay];
             // one upwinded product at a time: MP5 L/R (O3) of (vbar, B) to the edge, then O7
-            auto along_x = [&](int f, double ap, double am) {
-                const double *p = &sXR[ps][f][ty * UCT_XRW + tx], *q = p + UCT_XR;
+            auto bracket = [&](const double *p, const double *q, int S, double ap, double am) {
                 double vL, vR, BL, BR;
-                mp5_pair<false>(p[0], p[1], p[2], p[3], p[4], p[5], vL, vR);
-                mp5_pair<false>(q[0], q[1], q[2], q[3], q[4], q[5], BL, BR);
+                const unsigned nv = mp5_pair_fast(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+                const unsigned nb = mp5_pair_fast(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+                if (nv | nb) {
+                    mp5_pair_fix(nv, p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+                    mp5_pair_fix(nb, q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+                }
                 return uct_hll(ap, am, vL, vR, BL, BR);
+            };
+            auto along_x = [&](int f, double ap, double am) {
+                const double *p = &sXR[ps][f][ty * UCT_XRW + tx];
+                return bracket(p, p + UCT_XR, 1, ap, am);
             };
             auto along_y = [&](int f, double ap, double am) {
-                const double *p = &sYR[ps][f][ty * UCT_TX + tx], *q = p + UCT_YR;
-                constexpr int S = UCT_TX;
-                double vL, vR, BL, BR;
-                mp5_pair<false>(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
-                mp5_pair<false>(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
-                return uct_hll(ap, am, vL, vR, BL, BR);
+                const double *p = &sYR[ps][f][ty * UCT_TX + tx];
+                return bracket(p, p + UCT_YR, UCT_TX, ap, am);
             };
-            auto along_z = [&](int f, double ap, double am) {
-                const double *p = zw[f], *q = zw[f + 1];
-                double vL, vR, BL, BR;
-                mp5_pair<false>(p[0], p[1], p[2], p[3], p[4], p[5], vL, vR);
-                mp5_pair<false>(q[0], q[1], q[2], q[3], q[4], q[5], BL, BR);
-                return uct_hll(ap, am, vL, vR, BL, BR);
-            };
+            auto along_z = [&](int f, double ap, double am) { return bracket(zw[f], zw[f + 1], 1, ap, am); };
             // E_z: i = x, j = y
             const double ez = -along_x(0, dmax(axp, sAX[as0][0][iax + UCT_TX]), dmax(axm, sAX[as0][1][iax + UCT_TX])) +
                               along_y(0, dmax(ayp, sAY[as0][0][iay + 1]), dmax(aym, sAY[as0][1][iay + 1]));
