@@ -44,11 +44,8 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
     const double e = fma(-(x * y), y, 1.0);
     return fma(y * e, fma(0.375, e, 0.5), y);
 }
-__device__ __forceinline__ double sqrt_fast(double x) {   // x >= 0; exact 0 -> 0
-    const double y = rsqrt_fast(x);
-    const double s = x * y;
-    const double r = fma(-s, s, x);
-    const double t = fma(r, 0.5 * y, s);
+__device__ __forceinline__ double sqrt_fast(double x) {   // x >= 0; exact 0 -> 0; ~1-2 ulp (x * rsqrt(x))
+    const double t = x * rsqrt_fast(x);
     return x > 0.0 ? t : 0.0;
 }
 
@@ -214,19 +211,19 @@ __device__ __forceinline__ void side_state(double gam, double gg, const double q
     }
     f[1 + D] += fma(0.5, b2, p);
     f[4] = u[1 + D];
-    // O4: a^2 = cs^2 + ca^2 - cs^2 ca^2, cs^2 = gamma p/(rho h), ca^2 = b^2/(rho h + b^2)
+    // O4.  a^2 = cs^2 + ca^2 - cs^2 ca^2 with cs^2 = gamma p/(rho h), ca^2 = b^2/w, w = rho h + b^2 collapses to
+    // a^2 = A/w, A = gamma p + b^2.  Multiplying numerator and denominator of lambda+- by w:
+    //   lambda+- = [ (w - A) v_D +- sqrt( A (1-v^2) [ (w - v^2 A) - (w - A) v_D^2 ] ) ] / (w - v^2 A)
+    // — one square root and one reciprocal per side, no division.
     const double w = rhoh + b2;
-    const double r = rcp_fast(rhoh * w);
-    const double cs2 = gam * p * w * r;
-    const double ca2 = b2 * rhoh * r;
-    const double a2 = cs2 + ca2 - cs2 * ca2;
-    const double oma2 = 1.0 - a2;
-    const double den = 1.0 - v2 * a2;
+    const double A = fma(gam, p, b2);
+    const double N = fma(-v2, A, w);
+    const double M = w - A;
     const double vd = v[D];
-    const double root = sqrt_fast(a2 * omv2 * (den - oma2 * vd * vd));
-    const double rden = rcp_fast(den);
-    lp = (oma2 * vd + root) * rden;
-    lm = (oma2 * vd - root) * rden;
+    const double sq = sqrt_fast(A * omv2 * fma(-M, vd * vd, N));
+    const double rN = rcp_fast(N);
+    lp = fma(M, vd, sq) * rN;
+    lm = fma(M, vd, -sq) * rN;
 }
 
 // O5 — two-state HLL flux at a D-face; also the stored UCT pieces:
