@@ -135,6 +135,36 @@ int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host);
  * 1e-15 is measurable.  Synchronises.  Returns ECHO_EC2P if the failure count is non-zero. */
 int echo_diagnostics(echo_ctx *ctx, double *out);
 
+/* ---- domain-decomposition blocks ("next" row f1: multi-GPU) ----------------------------
+ * A block is a periodic box of nx*ny*nz cells INCLUDING halo_d cells on each side of every decomposed axis
+ * (halo_d = 0: the block spans the whole periodic axis), with the spacing h_d = 1/gn_d of the GLOBAL unit box of
+ * gnx*gny*gnz cells.  The kernels are the periodic ones of echo_step; the periodic wrap of the padded block only
+ * corrupts the halo, 8 cells per RK stage (the dependency reach of one stage, P:L138 + HO stencils), so with
+ * halo_d = 8 the interior stays exact provided the caller refreshes the halos of the 8 evolved fields from the
+ * neighbouring blocks after every stage.  a_max and the con2prim failure count only look at the interior.
+ * One step of a block, driven by the caller (paper_2401_03008_b200/blocks.py):
+ *     for stage in 1, 2, 3:
+ *         echo_stage_sweeps(ctx, stage, t_end)      INT + con2prim + the three sweeps (+ a_max in stage 1)
+ *         [stage 1: all-reduce(max) of the 8-byte a_max word at echo_ctrl_offset(0) across the blocks]
+ *         echo_stage_finish(ctx, stage)             (stage 1: dt) UCT, update of the stage's output fields
+ *         [refresh the halos of fields 8..15 (stages 1, 2) or 0..7 (stage 3) from the neighbours]
+ * echo_set_primitives / echo_get_primitives work on the padded block as on a plain box. */
+echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, int gnx, int gny, int gnz,
+                            int halo_x, int halo_y, int halo_z);
+
+/* Host only.  Byte offset, inside the workspace given to echo_bind, of field `field` (0..43; 0-7 the state U^n =
+ * D, Sx, Sy, Sz, U, Bx, By, Bz; 8-15 the stage state); each field is nx*ny*nz doubles. */
+size_t echo_field_offset(const echo_ctx *ctx, int field);
+
+/* Host only.  Byte offset inside the workspace of a control word: 0 = a_max as the bit pattern of a non-negative
+ * double (8 bytes, ordered like an unsigned integer: all-reduce it with MAX on int64), 1 = t, 2 = dt,
+ * 3 = con2prim failure count (uint64). */
+size_t echo_ctrl_offset(int what);
+
+/* First and second half of RK stage `stage` (1..3) of a block step; see above.  No synchronisation. */
+int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end);
+int echo_stage_finish(echo_ctx *ctx, int stage);
+
 /* ---- measurement aids (used by bench.py; not part of the numerical path) -------------------- */
 
 #define ECHO_NKCLASS 8

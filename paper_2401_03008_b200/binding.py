@@ -35,6 +35,11 @@ SIGNATURES = {
     "echo_prim2cons": (_int, [_dbl, _long] + [_vp] * 13 + [_vp]),
     "echo_div_b": (_int, [_vp, _vp, C.POINTER(_dbl)]),
     "echo_diagnostics": (_int, [_vp, C.POINTER(_dbl)]),
+    "echo_create_block": (_vp, [_int, _int, _int, _dbl, _dbl, _int, _int, _int, _int, _int, _int]),
+    "echo_field_offset": (_sz, [_vp, _int]),
+    "echo_ctrl_offset": (_sz, [_int]),
+    "echo_stage_sweeps": (_int, [_vp, _int, _dbl]),
+    "echo_stage_finish": (_int, [_vp, _int]),
     "echo_timing": (_int, [_vp, _int]),
     "echo_get_timing": (_int, [_vp, C.POINTER(_dbl), C.POINTER(_long)]),
     "echo_fp64_peak": (_int, [_int, C.POINTER(_dbl), _vp]),
@@ -93,14 +98,18 @@ class EchoError(RuntimeError):
 class Echo:
     """One periodic unit box on the current CUDA device.  Tensors are torch.float64, shape (nz, ny, nx)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, device=None):
+    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None):
+        """block = (gnx, gny, gnz, halo_x, halo_y, halo_z): a domain-decomposition block (echo_create_block)."""
         torch = _torch()
         self.L = lib()
         self.n = (nx, ny, nz)
         self.shape = (nz, ny, nx)
         self.N = nx * ny * nz
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
-        self.h = self.L.echo_create(nx, ny, nz, gamma, cfl)
+        if block is None:
+            self.h = self.L.echo_create(nx, ny, nz, gamma, cfl)
+        else:
+            self.h = self.L.echo_create_block(nx, ny, nz, gamma, cfl, *[int(b) for b in block])
         if not self.h:
             raise ValueError("echo_create: bad arguments")
         nbytes = self.L.echo_workspace_bytes(self.h)
@@ -181,6 +190,23 @@ class Echo:
         d["rc"] = rc
         return d
 
+
+    # ---- domain-decomposition blocks
+    def field(self, idx):
+        """Field idx (0..43) of the workspace as a (nz, ny, nx) float64 tensor VIEW (no copy)."""
+        off = self.L.echo_field_offset(self.h, int(idx))
+        return self.workspace[off:off + 8 * self.N].view(_torch().float64).view(self.shape)
+
+    def ctrl_word(self, what):
+        """8-byte control word as an int64 tensor view: 0 = a_max bits, 1 = t, 2 = dt, 3 = con2prim failures."""
+        off = self.L.echo_ctrl_offset(int(what))
+        return self.workspace[off:off + 8].view(_torch().int64)
+
+    def stage_sweeps(self, stage, t_end=math.inf):
+        self._check(self.L.echo_stage_sweeps(self.h, int(stage), float(t_end)))
+
+    def stage_finish(self, stage):
+        self._check(self.L.echo_stage_finish(self.h, int(stage)))
 
     # ---- measurement aids
     def timing(self, enable=True):

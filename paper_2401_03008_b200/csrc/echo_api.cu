@@ -1,6 +1,7 @@
 // echo_api.cu — C-ABI layer of libecho_b200 (see include/echo.h): argument checks, workspace
 // carving, kernel launches on the bound stream.  No arithmetic of the method lives here.
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -23,6 +24,7 @@ struct echo_ctx {
     double *field[NFIELD] = {nullptr};
     long long npad = 0;
     bool bound = false, has_state = false;
+    bool block = false;      // echo_create_block: explicit spacing, halos refreshed by the caller between stages
     std::string err;
     // measurement aids (echo_timing / echo_get_timing)
     bool timing = false;
@@ -128,8 +130,8 @@ struct StagePlan {
     double c0, c1;
 };
 
-// points 1-4 of a sub-step on the given stage pointers (P:L128-135)
-int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan *pl = nullptr) {
+// points 1-3 of a sub-step (INT + con2prim, the three sweeps) on the given stage pointers
+int launch_sweeps(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan *pl = nullptr) {
     const Grid &g = ctx->g;
     PrimUpd pu;
     for (int v = 0; v < 5; ++v) pu.uout[v] = ctx->field[F_U1 + v];
@@ -150,7 +152,13 @@ int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePl
     if ((rc = launch_flux<1, 0>(ctx, st, want_amax, fu))) return rc;
     if (pl && pl->fuse_z) { if ((rc = launch_flux<2, 1>(ctx, st, want_amax, fu))) return rc; }
     else                  { if ((rc = launch_flux<2, 0>(ctx, st, want_amax, fu))) return rc; }
-    if (want_amax == 2) {   // stage 1 of echo_step: dt must exist before any update (S9)
+    return ECHO_OK;
+}
+
+// k_set_dt (stage 1 only) + point 4 (UCT)
+int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
+    const Grid &g = ctx->g;
+    if (set_dt) {   // stage 1 of a step: dt must exist before any update (S9)
         KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
     }
     {   // plane-marching UCT: 16 x 8 tiles of (x, y), chunks of planes along z sized for >= ~8 blocks per SM
@@ -164,6 +172,13 @@ int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePl
         KL(KC_UCT, "k_uct2", k_uct2<<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
     }
     return ECHO_OK;
+}
+
+// points 1-4 of a sub-step on the given stage pointers (P:L128-135)
+int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan *pl = nullptr) {
+    int rc;
+    if ((rc = launch_sweeps(ctx, st, want_amax, pl))) return rc;
+    return launch_uct(ctx, st, want_amax == 2);
 }
 
 // curl + RK combination of the staggered B (and, with_u, of the 5 cell fields as well)
@@ -212,7 +227,7 @@ echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl) {
     g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
     g.s[0] = 1; g.s[1] = nx; g.s[2] = nx * ny;
     g.N = (long long)nx * ny * nz;
-    for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; }
+    for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; g.lo[d] = 0; g.hi[d] = g.n[d]; }
     c->gamma = gamma;
     c->cfl = cfl;
     c->gg = gamma / (gamma - 1.0);
@@ -480,6 +495,73 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
     out[17] = h.c2p_calls ? (double)h.c2p_sumit / (double)h.c2p_calls : 0.0;
     out[18] = (double)h.c2p_fail_total;
     return h.c2p_fail_total ? fail(ctx, ECHO_EC2P, "con2prim failed in at least one cell") : ECHO_OK;
+}
+
+// ---- domain-decomposition blocks
+echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, int gnx, int gny, int gnz, int halo_x,
+                            int halo_y, int halo_z) {
+    const int n[3] = {nx, ny, nz}, gn[3] = {gnx, gny, gnz}, hl[3] = {halo_x, halo_y, halo_z};
+    for (int d = 0; d < 3; ++d)
+        if (gn[d] < 1 || hl[d] < 0 || n[d] - 2 * hl[d] < 1 || (hl[d] > 0 && n[d] - 2 * hl[d] < hl[d])) return nullptr;
+    echo_ctx *c = echo_create(nx, ny, nz, gamma, cfl);
+    if (!c) return nullptr;
+    Grid &g = c->g;
+    for (int d = 0; d < 3; ++d) {
+        g.h[d] = 1.0 / gn[d];           // the spacing of the GLOBAL unit box, same arithmetic as echo_create
+        g.rh[d] = (double)gn[d];
+        g.lo[d] = hl[d];
+        g.hi[d] = n[d] - hl[d];
+    }
+    c->hmin = std::fmin(g.h[0], std::fmin(g.h[1], g.h[2]));
+    c->block = true;
+    return c;
+}
+
+size_t echo_field_offset(const echo_ctx *ctx, int field) {
+    if (!ctx || field < 0 || field >= NFIELD) return 0;
+    return CTRL_BYTES + PART_BYTES + sizeof(double) * (size_t)ctx->npad * field;
+}
+
+size_t echo_ctrl_offset(int what) {
+    switch (what) {
+        case 0: return offsetof(Ctrl, amax_bits);
+        case 1: return offsetof(Ctrl, t);
+        case 2: return offsetof(Ctrl, dt);
+        case 3: return offsetof(Ctrl, c2p_fail_total);
+        default: return (size_t)-1;
+    }
+}
+
+int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
+    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    if (stage == 1) {
+        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+        return launch_sweeps(ctx, s0, 2);
+    }
+    // stages 2, 3: the stage buffers hold the (halo-refreshed) state; RK combination fused into the z-sweep
+    const StagePlan pl2 = {false, true, 1, 1, 0.75, 0.25}, pl3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
+    return launch_sweeps(ctx, s1, 0, stage == 2 ? &pl2 : &pl3);
+}
+
+int echo_stage_finish(echo_ctx *ctx, int stage) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
+    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    if (stage == 1) {
+        // dt from the (all-reduced) a_max, UCT, then the UNFUSED update of all 8 fields: U1 must exist in
+        // memory for the halo refresh that precedes stage 2
+        if ((rc = launch_uct(ctx, s0, true))) return rc;
+        return launch_update(ctx, s0, 0, 1, 0.0, 1.0, true);
+    }
+    if ((rc = launch_uct(ctx, s1, false))) return rc;
+    if (stage == 2) return launch_update(ctx, s1, 1, 1, 0.75, 0.25, false);
+    if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false))) return rc;
+    KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+    return ECHO_OK;
 }
 
 int echo_timing(echo_ctx *ctx, int enable) {

@@ -96,7 +96,8 @@ __global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl
         for (int v = 0; v < 5; ++v) st.P[v][c] = q[v];
 #pragma unroll
         for (int d = 0; d < 3; ++d) st.Bc[d][c] = B[d];
-        if (it < 0) atomicAdd(&ctrl->c2p_fail_total, 1ull);
+        if (it < 0 && i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2])
+            atomicAdd(&ctrl->c2p_fail_total, 1ull);
     }
     if (STATS) {
         __shared__ int s_sum[8], s_max[8], s_cnt[8];
@@ -279,7 +280,10 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
                 st.am[D][o] = am;
                 st.vb[D][0][o] = vb1;
                 st.vb[D][1][o] = vb2;
-                amax = dmax(amax, dmax(ap, am));
+                const int cD = m0 + f - 3, cTT = t0 + b, cOO = (int)blockIdx.z;
+                const bool inner = cD >= g.lo[D] && cD < g.hi[D] && cTT >= g.lo[TD] && cTT < g.hi[TD] &&
+                                   cOO >= g.lo[OD] && cOO < g.hi[OD];
+                if (inner) amax = dmax(amax, dmax(ap, am));
             }
         }
 

@@ -10,6 +10,10 @@ struct Grid {
     int s[3];         // linear strides in elements: 1, nx, nx*ny (N < 2^31: 32-bit cell indices)
     long long N;
     double h[3], rh[3];   // spacing and its reciprocal (n_d exactly)
+    // interior of a domain-decomposition block (echo_create_block): cells lo_d <= c_d < hi_d; the rest is halo
+    // that the caller refreshes after every stage.  Global reductions (a_max, con2prim failures) only look at
+    // the interior.  A plain periodic box has lo = 0, hi = n.
+    int lo[3], hi[3];
 };
 
 // Device control block (first bytes of the workspace).  Everything echo_step needs between

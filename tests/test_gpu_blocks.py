@@ -1,0 +1,48 @@
+"""Row (f1): the domain-decomposed step (one padded periodic block per rank, halo refresh of the 8 evolved fields
+after every RK stage, all-reduce(max) of a_max) against the undecomposed run of the same library.  All blocks
+live in this process on one GPU (LocalBlocks): the same kernels, the same arithmetic per cell and an exact max,
+so the interiors must agree BIT FOR BIT; a wrong halo width, slab, corner or reduction shows up at once."""
+import numpy as np
+import pytest
+
+from paper_2401_03008_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+G = 4.0 / 3.0
+SETK = "rho vx vy vz p bxf byf bzf".split()
+
+
+@pytest.mark.parametrize("p", [(2, 1, 1), (1, 2, 2), (2, 2, 2), (1, 1, 3)])
+def test_blocks_match_single_domain_bitwise(p):
+    import torch
+    from paper_2401_03008_b200 import binding as eb, blocks
+    from oracle import binding as ob
+
+    gn = (32, 32, 48)
+    w = inputs.turbulence(None, shape=gn)
+    bo = ob.faces_from_potential(w["ax"], w["ay"], w["az"])
+    w["bxf"], w["byf"], w["bzf"] = [b + w["b0"][d] for d, b in enumerate(bo)]
+    e = eb.Echo(*gn, G, 0.3)
+    e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
+    lb = blocks.LocalBlocks(gn, p, G, 0.3)
+    lb.set_primitives(w)
+    t_end = 2.5 * 0.3 / 48 / 0.9          # inside the third step: exercises the clipped dt on every block
+    e.step(4, t_end)
+    lb.step(4, t_end)
+    d = e.diagnostics()
+    assert d["steps"] == 3 and lb.time() == d["t"] == t_end
+    q = {k: v.cpu().numpy() for k, v in e.get_primitives().items()}
+    qb = lb.get_primitives()
+    for k in q:
+        assert np.array_equal(q[k], qb[k]), (p, k, np.abs(q[k] - qb[k]).max())
+
+
+def test_block_argument_checks():
+    from paper_2401_03008_b200 import binding as eb, blocks
+    L = eb.lib()
+    assert not L.echo_create_block(20, 8, 8, G, 0.3, 32, 8, 8, 8, 0, 0)      # 4 interior cells < halo
+    assert not L.echo_create_block(16, 8, 8, G, 0.3, 0, 8, 8, 0, 0, 0)
+    with pytest.raises(ValueError):
+        blocks.Decomposition((30, 32, 32), (4, 1, 1))                        # 30 % 4 != 0
+    with pytest.raises(ValueError):
+        blocks.Decomposition((32, 32, 32), (8, 1, 1))                        # 4 cells per block < halo
