@@ -18,13 +18,19 @@ TWO_PI = 2.0 * math.pi
 
 # --------------------------------------------------------------------------------------
 # grid helpers: unit periodic box, cell (i,j,k) centred at ((i+1/2)hx, ...)
-def _coords(n, offset):
-    return (np.arange(n, dtype=np.float64) + offset) / n
+def _coords(n, offset, start=0, gn=None):
+    """(start + i + offset)/gn for i < n: the same expression whether a whole box (start = 0, gn = n) or a block
+    of a larger box is sampled, so a block carries bit-identical values to the corresponding part of the box."""
+    gn = n if gn is None else gn
+    i = (np.arange(n, dtype=np.int64) + int(start)) % int(gn)
+    return (i.astype(np.float64) + offset) / gn
 
 
-def _mesh(nx, ny, nz, ox, oy, oz):
-    """Coordinates of points displaced by (ox,oy,oz) cells from the cell corner, shape (nz,ny,nx)."""
-    z, y, x = np.meshgrid(_coords(nz, oz), _coords(ny, oy), _coords(nx, ox), indexing="ij")
+def _mesh(nx, ny, nz, ox, oy, oz, box=None):
+    """Coordinates of points displaced by (ox,oy,oz) cells from the cell corner, shape (nz,ny,nx).
+    box = ((gnx, gny, gnz), (sx, sy, sz)): the nx*ny*nz cells starting at (sx, sy, sz) of a periodic gn box."""
+    (gx, gy, gz), (sx, sy, sz) = box if box is not None else ((nx, ny, nz), (0, 0, 0))
+    z, y, x = np.meshgrid(_coords(nz, oz, sz, gz), _coords(ny, oy, sy, gy), _coords(nx, ox, sx, gx), indexing="ij")
     return x, y, z
 
 
@@ -65,18 +71,19 @@ def cpa_period(direction="diag", **kw):
     return TWO_PI / (np.linalg.norm(kvec) * vA)
 
 
-def cpa_wave(nx, ny, nz, t=0.0, direction="diag", rho=1.0, p=1.0, B0=1.0, eta=1.0, gamma=4.0 / 3.0):
+def cpa_wave(nx, ny, nz, t=0.0, direction="diag", rho=1.0, p=1.0, B0=1.0, eta=1.0, gamma=4.0 / 3.0, box=None):
     """Exact CPA-wave fields at time t (phase k.x - |k| vA t).
 
     Returns a dict: rho, vx, vy, vz, p, bx, by, bz at cell centres; bxf, byf, bzf analytic
     point values at the staggered faces; vA, T (period), kvec.
+    box = ((gnx, gny, gnz), (sx, sy, sz)) samples a block of a larger periodic box (domain decomposition).
     """
     X, Y, Z, kvec = _cpa_frame(direction)
     vA = alfven_speed(rho, p, B0, eta, gamma)
     kmod = float(np.linalg.norm(kvec))
 
     def fields(off):
-        x, y, z = _mesh(nx, ny, nz, *off)
+        x, y, z = _mesh(nx, ny, nz, *off, box=box)
         phi = kvec[0] * x + kvec[1] * y + kvec[2] * z - kmod * vA * t
         c, s = np.cos(phi), np.sin(phi)
         dB = [eta * B0 * (c * Y[a] + s * Z[a]) for a in range(3)]

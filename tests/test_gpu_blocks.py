@@ -46,3 +46,30 @@ def test_block_argument_checks():
         blocks.Decomposition((30, 32, 32), (4, 1, 1))                        # 30 % 4 != 0
     with pytest.raises(ValueError):
         blocks.Decomposition((32, 32, 32), (8, 1, 1))                        # 4 cells per block < halo
+
+
+def test_rank_block_world_of_one():
+    """RankBlock (the torch.distributed driver) in a world of one rank: NCCL all-reduce of the a_max word, no
+    exchange; must reproduce the plain run bit for bit."""
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_2401_03008_b200 import binding as eb, blocks
+
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29755")
+    dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        gn = (24, 16, 20)
+        w = inputs.cpa_wave(*gn)
+        e = eb.Echo(*gn, G, 0.3)
+        e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
+        rb = blocks.RankBlock(gn, (1, 1, 1), G, 0.3)
+        rb.set_primitives(w)
+        e.step(3)
+        rb.step(3)
+        q, qb = e.get_primitives(), rb.get_interior()
+        for k in q:
+            assert torch.equal(q[k], qb[k]), k
+    finally:
+        dist.destroy_process_group()
