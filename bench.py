@@ -188,6 +188,16 @@ def run_gpu(args):
         e = rb.block
         stepper = rb.step
         parallelism = "one box of %dx%dx%d cells in %dx%dx%d blocks, halo 8, NCCL p2p + all-reduce(max)" % (gn + pgrid)
+    elif args.workload == "turb2d":
+        # row f3: the paper's 2.5-D turbulence set-up on an n x n x 1 grid; faces from the potential
+        w = inputs.turbulence_2d(n)
+        N = n * n
+        e = binding.Echo(n, n, 1, GAMMA, CFL)
+        faces = e.faces_from_potential(*[torch.as_tensor(w[k], device="cuda") for k in ("ax", "ay", "az")], w["b0"])
+        for k, f in zip(("bxf", "byf", "bzf"), faces):
+            w[k] = f.cpu().numpy()
+        stepper = e.step
+        parallelism = "replicas x%d (no collective)" % world
     else:
         w = inputs.cpa_wave(n, n, n, direction=args.direction)
         e = binding.Echo(n, n, n, GAMMA, CFL)
@@ -239,7 +249,7 @@ def run_gpu(args):
     barrier()
     e2e_value, _ = whole_job_rate(N, Ke, ev0.elapsed_time(ev1), "cuda", world)
     # sanity of what came back: one step of the wave stays within truncation error of the input
-    assert abs(float(outs[0].mean()) - 1.0) < 1e-6
+    assert abs(float(outs[0].mean()) - 1.0) < (1e-6 if args.workload == "cpa" else 1e-2)
 
     if rank != 0:
         if world > 1:
@@ -285,7 +295,8 @@ def run_gpu(args):
     line = {"metric": "fp64_cell_updates_per_sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "cpa_wave_%s_%d^3" % (args.direction, n), "grid": [n, n, n], "gamma": GAMMA, "cfl": CFL,
+            "config": {"workload": ("turbulence_2.5d_%d^2" % n) if args.workload == "turb2d" else "cpa_wave_%s_%d^3" % (args.direction, n),
+                       "grid": list(e.n), "gamma": GAMMA, "cfl": CFL,
                        "scheme": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)", "cells": N,
                        "parallelism": parallelism,
                        "cache": "working set %.1f GB per GPU, far larger than the 126 MB L2" % (44 * 8 * N / 1e9)},
@@ -326,6 +337,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=6)
     ap.add_argument("--ref-n", type=int, default=48)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--workload", default="cpa", choices=["cpa", "turb2d"],
+                    help="cpa: BASELINE.json configs (default); turb2d: the paper's 2.5-D turbulence on n x n x 1")
     ap.add_argument("--decompose", action="store_true",
                     help="N > 1: one decomposed box (n^3 cells per rank, halo exchange) instead of N replicas")
     args = ap.parse_args()

@@ -114,6 +114,11 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
     constexpr int NT = FLUX_NT, T = (D == 0) ? 4 : 16;
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
+    if (g.n[D] == 1) {   // a one-cell axis: no stencil work left, only the face quantities (k_flux_flat)
+        KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
+               g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        return ECHO_OK;
+    }
     // chunks along D: one chunk per column unless the axis is long (5 halo faces per chunk are recomputed)
     const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
     const int C = (g.n[D] + nchunk - 1) / nchunk;

@@ -323,6 +323,57 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
     }
 }
 
+// k_flux_flat: the sweep along an axis of ONE cell (2.5-D / 1.5-D runs through the periodic wrap).  All faces of
+// a column are the same face, so the DER + difference of point 3 vanishes identically (rhs unchanged) and only the
+// face quantities UCT needs (a+, a-, vbar), a_max and, in MODE 1, the RK combination remain.  The arithmetic of
+// the face is the generic one applied to six equal stencil values, so a flat run stays bit-identical to the same
+// data on a thicker grid (dimensional-reduction test).
+template <int D, int MODE>
+__global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam, double gg, Ctrl *ctrl, int want_amax,
+                                                   FluxUpd up) {
+    constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    double amax = 0.0;
+    if (i < g.n[0] && j < g.n[1]) {
+        const int c = i + g.s[1] * j + g.s[2] * k;
+        const double *rec[7] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2]};
+        constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+        double qL[8], qR[8];
+#pragma unroll
+        for (int v = 0; v < 7; ++v) {
+            const double s = __ldg(rec[v] + c);
+            mp5_pair<true>(s, s, s, s, s, s, qL[slot[v]], qR[slot[v]]);
+        }
+        qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + c);
+        double F[5], ap, am, vb1, vb2;
+        hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
+        st.ap[D][c] = ap;
+        st.am[D][c] = am;
+        st.vb[D][0][c] = vb1;
+        st.vb[D][1][c] = vb2;
+        const bool inner = i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2];
+        if (inner) amax = dmax(ap, am);
+        if (MODE == 1) {
+            const double dt = ctrl->dt;
+            if (ctrl->active) {
+#pragma unroll
+                for (int v = 0; v < 5; ++v)
+                    up.out[v][c] = up.c0 * __ldg(up.base[v] + c) + up.c1 * (up.cur[v][c] + dt * __ldg(st.R[v] + c));
+            }
+        } else if (D == 0) {
+#pragma unroll
+            for (int v = 0; v < 5; ++v) st.R[v][c] = 0.0;     // the x-sweep is the one that initialises rhs
+        }
+    }
+    if (want_amax) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) amax = dmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        if (((threadIdx.y * blockDim.x + threadIdx.x) & 31) == 0 && amax > 0.0) atomic_max_nonneg(&ctrl->amax_bits, amax);
+    }
+}
+
 }  // namespace echo
 #include "echo_uct.cuh"   // k_uct2: the plane-marching UCT kernel used by echo_step
 namespace echo {

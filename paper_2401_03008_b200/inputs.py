@@ -182,6 +182,52 @@ def turbulence(n, seed=2401, rho0=1.0, p0=0.1, sigma=1.0, amp=0.5, gamma=4.0 / 3
 
 
 # --------------------------------------------------------------------------------------
+# 2.5-D decaying RMHD turbulence of the paper, eq.(13)-(17)  (row f3)
+def turbulence_2d(nx, ny=None, seed=2401, eta_mean=0.25, gamma=4.0 / 3.0):
+    """The paper's own turbulence set-up on an nx x ny x 1 grid (fluctuations in the x-y plane, B0 along z).
+
+    rho0 = 1, sigma0 = B0^2/rho0 = 100, beta0 = 2 p0/B0^2 = 1  =>  B0 = 10, p0 = 50 (eq.(13), P:L311-313);
+    vA = B0/sqrt(rho0 + 4 p0 + B0^2) (eq.(14)); modes m = (mx, my), mx = 0..4, my = -4..4 (eq.(15)-(16)),
+    kept when 1 <= |m| <= 4 ("spectral radius of 4") and, for mx = 0, my > 0 (the conjugate would be the
+    same mode); delta v = eta vA sum (m x e_z)/|m| cos(2 pi m.x + phi_v), delta B likewise with B0 and phi_B,
+    independent random phases (splitmix64(seed), B phases first); the staggered delta B comes from the potential
+    a_z = sum sin(2 pi m.x + phi_B)/(2 pi |m|) at the z-edges, curled by the solver under test (S11).  eta is
+    fixed a posteriori so that the MEAN magnitudes satisfy <|dv|>/vA = <|dB|>/B0 = eta_mean (eq.(17), read
+    literally; |dB| is evaluated from the analytic field at the cell centres).  The paper's box has L = 2 pi; the
+    equations have no length scale, so the unit box is used and one paper time unit is 1/(2 pi) here.
+    """
+    ny = nx if ny is None else ny
+    rho0, B0 = 1.0, 10.0
+    p0 = 0.5 * B0 * B0
+    vA = B0 / math.sqrt(rho0 + gamma / (gamma - 1.0) * p0 + B0 * B0)
+    modes = [(mx, my) for mx in range(0, 5) for my in range(-4, 5)
+             if 1 <= mx * mx + my * my <= 16 and (mx > 0 or my > 0)]
+    rng = SplitMix64(seed)
+    phB = [TWO_PI * rng.uniform() for _ in modes]
+    phV = [TWO_PI * rng.uniform() for _ in modes]
+    xc, yc, _ = _mesh(nx, ny, 1, *CENTRE)
+    xe, ye, _ = _mesh(nx, ny, 1, *EDGE[2])
+    sh = (1, ny, nx)
+    vx, vy, bxc, byc, az = (np.zeros(sh) for _ in range(5))
+    for (mx, my), pb, pv in zip(modes, phB, phV):
+        km = math.sqrt(mx * mx + my * my)
+        cv = np.cos(TWO_PI * (mx * xc + my * yc) + pv)
+        cb = np.cos(TWO_PI * (mx * xc + my * yc) + pb)
+        vx += (my / km) * cv
+        vy += (-mx / km) * cv
+        bxc += (my / km) * cb
+        byc += (-mx / km) * cb
+        az += np.sin(TWO_PI * (mx * xe + my * ye) + pb) / (TWO_PI * km)
+    sv = eta_mean / float(np.sqrt(vx * vx + vy * vy).mean())
+    sb = eta_mean / float(np.sqrt(bxc * bxc + byc * byc).mean())
+    full = lambda v: np.full(sh, v)
+    return {"rho": full(rho0), "p": full(p0), "vx": sv * vA * vx, "vy": sv * vA * vy, "vz": full(0.0),
+            "ax": full(0.0), "ay": full(0.0), "az": sb * B0 * az, "b0": (0.0, 0.0, B0),
+            "B0": B0, "vA": vA, "gamma": gamma, "modes": modes,
+            "vmax": float(sv * vA * np.sqrt(vx * vx + vy * vy).max())}
+
+
+# --------------------------------------------------------------------------------------
 def random_states(n, seed=12345, gamma=4.0 / 3.0, wmax=10.0, sigma_max=10.0):
     """P6 sample: random primitive states up to Lorentz factor wmax and magnetisation sigma_max.
 

@@ -286,3 +286,22 @@ def test_error_codes(torch, eb):
     with pytest.raises(eb.EchoError) as ei:
         e.step(1)                                                  # bound, but no state yet
     assert ei.value.code == eb.ECHO_ESTATE
+
+
+def test_turbulence_2d_paper_setup(torch, eb, ob):
+    """Row f3: the paper's own 2.5-D turbulence set-up (eq.(13)-(17): sigma0 = 100, beta0 = 1, 24 in-plane
+    Alfvenic modes, <|dv|>/vA = <|dB|>/B0 = 0.25) on a 64 x 48 x 1 grid: the size-1 axis runs through the same
+    kernels; 10 steps against the oracle, div B at round-off."""
+    shape = (64, 48, 1)
+    w = inputs.turbulence_2d(64, 48)
+    bo = ob.faces_from_potential(w["ax"], w["ay"], w["az"])
+    w["bxf"], w["byf"], w["bzf"] = [b + w["b0"][d] for d, b in enumerate(bo)]
+    assert abs(np.sqrt(w["vx"] ** 2 + w["vy"] ** 2).mean() / w["vA"] - 0.25) < 1e-12          # eq.(17)
+    assert w["vA"] == pytest.approx(0.57639, abs=1e-5)                                         # eq.(14): "~0.57"
+    e, o = make_pair(torch, eb, ob, w, shape)
+    e.step(10)
+    o.step(10)
+    compare_prims(e, o, tight=1e-11)
+    dg, do = e.diagnostics(), o.diagnostics()
+    assert dg["t"] == pytest.approx(do["t"], rel=1e-13) and dg["c2p_failures"] == 0
+    assert dg["max_div_b"] <= 1e-12 * w["B0"] * 64 * 50
