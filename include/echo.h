@@ -98,6 +98,16 @@ int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy,
                              double *p, double *bx_c, double *by_c, double *bz_c, double *bx_face,
                              double *by_face, double *bz_face);
 
+/* Same, without the final synchronisation: the host buffers (which must be PINNED for the copies to be
+ * asynchronous) are valid after echo_synchronize(ctx).  Lets a caller overlap the transfers of one handle with
+ * the kernels of another handle bound to a different stream. */
+int echo_get_primitives_host_async(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz,
+                                   double *p, double *bx_c, double *by_c, double *bz_c, double *bx_face,
+                                   double *by_face, double *bz_face);
+
+/* Blocks the host until everything enqueued on the handle's stream has finished. */
+int echo_synchronize(echo_ctx *ctx);
+
 /* Copies the 5 conserved cell fields D, Sx, Sy, Sz, U of the current state (device). */
 int echo_get_conserved(echo_ctx *ctx, double *D, double *Sx, double *Sy, double *Sz, double *U);
 

@@ -29,6 +29,8 @@ SIGNATURES = {
     "echo_step": (_int, [_vp, _int, _dbl]),
     "echo_get_primitives": (_int, [_vp] + [_vp] * 11),
     "echo_get_primitives_host": (_int, [_vp] + [_vp] * 11),
+    "echo_get_primitives_host_async": (_int, [_vp] + [_vp] * 11),
+    "echo_synchronize": (_int, [_vp]),
     "echo_get_conserved": (_int, [_vp] + [_vp] * 5),
     "echo_rhs": (_int, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_dbl)]),
     "echo_con2prim": (_int, [_dbl, _long] + [_vp] * 13 + [_vp, _vp]),
@@ -157,10 +159,14 @@ class Echo:
         names = ["rho", "vx", "vy", "vz", "p", "bx", "by", "bz", "bxf", "byf", "bzf"]
         return dict(zip(names, out))
 
-    def get_primitives_host(self, outs):
-        """outs: 8 or 11 host FP64 buffers; synchronises."""
+    def get_primitives_host(self, outs, sync=True):
+        """outs: 8 or 11 host FP64 buffers; synchronises unless sync=False (then call synchronize())."""
         ptrs = [_host_ptr(a, self.N) for a in outs] + [None] * (11 - len(outs))
-        self._check(self.L.echo_get_primitives_host(self.h, *ptrs))
+        fn = self.L.echo_get_primitives_host if sync else self.L.echo_get_primitives_host_async
+        self._check(fn(self.h, *ptrs))
+
+    def synchronize(self):
+        self._check(self.L.echo_synchronize(self.h))
 
     def get_conserved(self):
         out = self._new(5)

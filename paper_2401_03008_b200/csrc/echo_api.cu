@@ -365,8 +365,9 @@ int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, doub
     return ECHO_OK;
 }
 
-int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p, double *bxc,
-                             double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
+static int get_primitives_host_impl(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p,
+                                    double *bxc, double *byc, double *bzc, double *bxf, double *byf, double *bzf,
+                                    bool sync) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     if (!rho || !vx || !vy || !vz || !p || !bxc || !byc || !bzc) return fail(ctx, ECHO_EINVAL, "null array");
@@ -379,6 +380,23 @@ int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy,
     double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d)
         if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], nb, cudaMemcpyDeviceToHost, ctx->stream));
+    if (sync) CU(cudaStreamSynchronize(ctx->stream));
+    return ECHO_OK;
+}
+
+int echo_get_primitives_host(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p, double *bxc,
+                             double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
+    return get_primitives_host_impl(ctx, rho, vx, vy, vz, p, bxc, byc, bzc, bxf, byf, bzf, true);
+}
+
+int echo_get_primitives_host_async(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p,
+                                   double *bxc, double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
+    return get_primitives_host_impl(ctx, rho, vx, vy, vz, p, bxc, byc, bzc, bxf, byf, bzf, false);
+}
+
+int echo_synchronize(echo_ctx *ctx) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
     CU(cudaStreamSynchronize(ctx->stream));
     return ECHO_OK;
 }

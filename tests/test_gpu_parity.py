@@ -305,3 +305,22 @@ def test_turbulence_2d_paper_setup(torch, eb, ob):
     dg, do = e.diagnostics(), o.diagnostics()
     assert dg["t"] == pytest.approx(do["t"], rel=1e-13) and dg["c2p_failures"] == 0
     assert dg["max_div_b"] <= 1e-12 * w["B0"] * 64 * 50
+
+
+def test_async_host_readback_two_streams(torch, eb, ob):
+    """echo_get_primitives_host_async + echo_synchronize on two handles bound to two streams (the pipelined
+    end-to-end path of bench.py) return exactly what the synchronous call returns."""
+    shape = (24, 16, 12)
+    w = turb_inputs(torch, eb, ob, None, shape=shape)
+    host = [torch.from_numpy(np.ascontiguousarray(w[k])).pin_memory() for k in SETK]
+    a = eb.Echo(*shape, G, 0.3)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        b = eb.Echo(*shape, G, 0.3)
+    oa = [torch.empty(shape[::-1], dtype=torch.float64).pin_memory() for _ in range(8)]
+    ob_ = [torch.empty(shape[::-1], dtype=torch.float64).pin_memory() for _ in range(8)]
+    a.set_primitives_host(*host); a.step(2); a.get_primitives_host(oa)
+    b.set_primitives_host(*host); b.step(2); b.get_primitives_host(ob_, sync=False)
+    b.synchronize()
+    for x, y in zip(oa, ob_):
+        assert torch.equal(x, y)
