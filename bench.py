@@ -188,6 +188,16 @@ def run_gpu(args):
         e = rb.block
         stepper = rb.step
         parallelism = "one box of %dx%dx%d cells in %dx%dx%d blocks, halo 8, NCCL p2p + all-reduce(max)" % (gn + pgrid)
+    elif args.workload == "turb3d":
+        # BASELINE.json configs[4]: relativistic Alfvenic turbulence on n^3 (384^3), sigma = 1, dB/B0 = 0.5
+        w = inputs.turbulence(n)
+        e = binding.Echo(n, n, n, GAMMA, CFL)
+        faces = e.faces_from_potential(*[torch.as_tensor(w[k], device="cuda") for k in ("ax", "ay", "az")], w["b0"])
+        for k, f in zip(("bxf", "byf", "bzf"), faces):
+            w[k] = f.cpu().numpy()
+        del faces
+        stepper = e.step
+        parallelism = "replicas x%d (no collective)" % world
     elif args.workload == "turb2d":
         # row f3: the paper's 2.5-D turbulence set-up on an n x n x 1 grid; faces from the potential
         w = inputs.turbulence_2d(n)
@@ -324,7 +334,8 @@ def run_gpu(args):
     line = {"metric": "fp64_cell_updates_per_sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": ("turbulence_2.5d_%d^2" % n) if args.workload == "turb2d" else "cpa_wave_%s_%d^3" % (args.direction, n),
+            "config": {"workload": {"turb2d": "turbulence_2.5d_%d^2" % n, "turb3d": "alfvenic_turbulence_%d^3" % n}.get(
+                           args.workload, "cpa_wave_%s_%d^3" % (args.direction, n)),
                        "grid": list(e.n), "gamma": GAMMA, "cfl": CFL,
                        "scheme": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)", "cells": N,
                        "parallelism": parallelism,
@@ -342,7 +353,9 @@ def run_gpu(args):
                               "achieved_tflops": per_gpu * FLOP_PER_CELL_UPDATE * 1e-12,
                               "achieved_gbs": per_gpu * BYTES_PER_CELL_UPDATE * 1e-9},
             "kernels": kernels,
-            "state": {"t": d["t"], "max_div_b": d["max_div_b"], "c2p_mean_iters": d["c2p_mean_iters"]},
+            "state": {"t": d["t"], "max_div_b": d["max_div_b"], "c2p_mean_iters": d["c2p_mean_iters"],
+                      "c2p_max_iters": d["c2p_max_iters"], "c2p_failures": d["c2p_failures"], "max_W": d["max_W"],
+                      "min_rho": d["min_rho"], "min_p": d["min_p"]},
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -367,7 +380,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=6)
     ap.add_argument("--ref-n", type=int, default=48)
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--workload", default="cpa", choices=["cpa", "turb2d"],
+    ap.add_argument("--workload", default="cpa", choices=["cpa", "turb2d", "turb3d"],
                     help="cpa: BASELINE.json configs (default); turb2d: the paper's 2.5-D turbulence on n x n x 1")
     ap.add_argument("--decompose", action="store_true",
                     help="N > 1: one decomposed box (n^3 cells per rank, halo exchange) instead of N replicas")
