@@ -317,7 +317,8 @@ def run_gpu(args):
                 "frac": kd["tflops"] / fp64_sust}
     else:
         roof = {"bound": "hbm", "achieved": kd["gbs"], "peak": hbm_peak, "unit": "GB/s", "frac": kd["gbs"] / hbm_peak}
-    roof.update(kernel=dom, traffic=TRAFFIC.get(dom), peak_source=("FP64 DFMA micro-benchmark run by this bench "
+    roof.update(kernel=dom, traffic=(TRAFFIC_PER_CELL[dom] * N if dom in TRAFFIC_PER_CELL else None),
+                traffic_source="ncu dram bytes per cell of profiles/r1_ncu_full.md (256^3, stage 2) x cells of this launch", peak_source=("FP64 DFMA micro-benchmark run by this bench "
                 "(sustained; burst %.1f)" % fp64_burst) if roof["bound"] == "alu" else "MEASURED_PEAKS.json (%s)" % peak_kind,
                 algorithmic_flop_per_cell=ALGO[dom]["flop"], algorithmic_bytes_per_cell=8 * ALGO[dom]["dbl"],
                 ms_per_launch=kd["ms_avg"], cells_per_launch=N)
@@ -362,9 +363,10 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/), keyed by kernel class; None until a capture of the current kernels exists.
-TRAFFIC = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch and per CELL from the committed ncu --set full capture
+# (profiles/r1_ncu_full.md: 256^3, RK stage 2), keyed by kernel class; bench.py reports it times the cells of a launch.
+TRAFFIC_PER_CELL = {"k_prim": 205.7, "k_flux_x": 135.2, "k_flux_y": 177.3, "k_flux_z": 258.4, "k_uct": 162.0,
+                    "k_update": 95.8}
 
 
 def main():
