@@ -1,8 +1,9 @@
 // echo_kernels.cuh — the kernels of one Runge-Kutta sub-step, sm_100a, FP64.
 //   k_prim      point 1: INT of the staggered B + con2prim                    (a1, a2)
 //   k_flux<D>   points 2+3: REC -> L/R -> HLL flux -> DER + divergence  (a3, a4, a8)
-//   k_uct       point 4: UCT edge EMFs                                        (a5)
-//   k_update    point 4b + 5 (eq.(10)): curl of DER(E) + RK combination (a6, a7)
+//   k_uct2      point 4: UCT edge EMFs (echo_uct.cuh, with k_bupd: curl + B update)   (a5, a6)
+//   k_update    point 4b + 5 (eq.(10)): curl + RK combination of all 8 fields; used for the
+//               unfused stage-1 update of block mode, k_bupd/k_prim<UPD>/k_flux<MODE 1> otherwise   (a6, a7)
 // plus the small control kernels that keep t, dt and a_max on the device.
 #pragma once
 #include "echo_math.cuh"
@@ -377,58 +378,6 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
 }  // namespace echo
 #include "echo_uct.cuh"   // k_uct2: the plane-marching UCT kernel used by echo_step
 namespace echo {
-
-// ------------------------------------------------------------------ point 4: UCT edge EMFs (O7) — reference form
-// (one thread per cell, every stencil through L1/L2; kept for grids whose x-y plane is tiny)
-// One thread per cell computes the three edge EMFs attached to it.  For the k-edge, with
-// i = (k+1)%3, j = (k+2)%3:   E_k = -HLL_i[ vbar_i B_j ] + HLL_j[ vbar_j B_i ]
-// where (vbar_i saved at j-faces, staggered B_j) are MP5-reconstructed along i and the edge speeds
-// are the max of the saved face speeds over the two faces adjacent to the edge.
-template <int K>
-__device__ __forceinline__ double uct_edge(const Stage &st, const int (*ix)[6], int c) {
-    constexpr int I = (K + 1) % 3, J = (K + 2) % 3;
-    // slots: direction J saves vbar_{(J+1)%3} = vbar_K in [0], vbar_{(J+2)%3} = vbar_I in [1];
-    //        direction I saves vbar_{(I+1)%3} = vbar_J in [0]
-    // q = 0: vbar_i along i, 1: B_j along i, 2: vbar_j along j, 3: B_i along j
-    const double *fld[4] = {st.vb[J][1], st.Bf[J], st.vb[I][0], st.Bf[I]};
-    double L[4], R[4];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int *x = ix[q < 2 ? I : J];
-        double s[6];
-#pragma unroll
-        for (int m = 0; m < 6; ++m) s[m] = __ldg(fld[q] + x[m]);
-        L[q] = mp5(s[0], s[1], s[2], s[3], s[4]);
-        R[q] = mp5(s[5], s[4], s[3], s[2], s[1]);
-    }
-    const int cj = ix[J][3], ci = ix[I][3];   // neighbours +1 along j and along i
-    const double aip = dmax(__ldg(st.ap[I] + c), __ldg(st.ap[I] + cj));
-    const double aim = dmax(__ldg(st.am[I] + c), __ldg(st.am[I] + cj));
-    const double ajp = dmax(__ldg(st.ap[J] + c), __ldg(st.ap[J] + ci));
-    const double ajm = dmax(__ldg(st.am[J] + c), __ldg(st.am[J] + ci));
-    const double viL = L[0], viR = R[0], BjL = L[1], BjR = R[1], vjL = L[2], vjR = R[2], BiL = L[3], BiR = R[3];
-    return -(aip * viL * BjL + aim * viR * BjR - aip * aim * (BjR - BjL)) * rcp_fast(aip + aim) +
-           (ajp * vjL * BiL + ajm * vjR * BiR - ajp * ajm * (BiR - BiL)) * rcp_fast(ajp + ajm);
-}
-
-__global__ void __launch_bounds__(256) k_uct(Grid g, Stage st) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
-    if (i >= g.n[0] || j >= g.n[1]) return;
-    const int c3[3] = {i, j, k};
-    const int c = i + g.s[1] * j + g.s[2] * k;
-    int ix[3][6];   // cells c-2 .. c+3 along each axis
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const int base = c - g.s[d] * c3[d];
-#pragma unroll
-        for (int m = 0; m < 6; ++m) ix[d][m] = base + g.s[d] * wrapi(c3[d] + m - 2, g.n[d]);
-    }
-    st.E[0][c] = uct_edge<0>(st, ix, c);
-    st.E[1][c] = uct_edge<1>(st, ix, c);
-    st.E[2][c] = uct_edge<2>(st, ix, c);
-}
 
 // ------------------------------------------------------------------ points 4b + 5: curl + RK update
 // rhs of the staggered B (O8, eq.(10)): dB_i/dt = -[ D_j(DER_j E_k) - D_k(DER_k E_j) ],
