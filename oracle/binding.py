@@ -39,6 +39,8 @@ def lib():
         L.oracle_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double]
         L.oracle_destroy.argtypes = [C.c_void_p]
         L.oracle_destroy.restype = None
+        L.oracle_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.oracle_faces_from_potential_ho.argtypes = [C.c_int] * 4 + [_dp] * 6
         L.oracle_set_primitives.argtypes = [C.c_void_p] + [_dp] * 8
         L.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.oracle_get_primitives.argtypes = [C.c_void_p] + [_dp] * 11
@@ -82,13 +84,18 @@ DIAG_NAMES = ["t", "dt_last", "steps", "amax", "sum_D", "sum_Sx", "sum_Sy", "sum
 class Oracle:
     """One periodic unit box.  Arrays are numpy float64 of shape (nz, ny, nx) (x fastest)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl):
+    def __init__(self, nx, ny, nz, gamma, cfl, uct=True, ho=True):
+        """uct / ho: the paper's scheme switches.  With uct=False the three B arrays given to
+        set_primitives (and returned as bxf, byf, bzf) are CELL-CENTRED."""
         self.L = lib()
         self.shape = (nz, ny, nx)
         self.n = (nx, ny, nz)
         self.h = self.L.oracle_create(nx, ny, nz, gamma, cfl)
         if not self.h:
             raise ValueError("oracle_create: bad arguments")
+        if not (uct and ho):
+            rc = self.L.oracle_set_scheme(self.h, int(bool(uct)), int(bool(ho)))
+            assert rc == 0, rc
 
     def __del__(self):
         if getattr(self, "h", None):
@@ -173,11 +180,14 @@ def prim2cons(gamma, rho, vx, vy, vz, p, Bx, By, Bz):
     return dict(D=outs[0], Sx=outs[1], Sy=outs[2], Sz=outs[3], U=outs[4])
 
 
-def faces_from_potential(ax, ay, az):
+def faces_from_potential(ax, ay, az, ho=True):
     a = [_c(x) for x in (ax, ay, az)]
     nz, ny, nx = a[0].shape
     out = [np.empty_like(a[0]) for _ in range(3)]
-    rc = lib().oracle_faces_from_potential(nx, ny, nz, *[_p(x) for x in a], *[_p(x) for x in out])
+    if ho:
+        rc = lib().oracle_faces_from_potential(nx, ny, nz, *[_p(x) for x in a], *[_p(x) for x in out])
+    else:
+        rc = lib().oracle_faces_from_potential_ho(nx, ny, nz, 0, *[_p(x) for x in a], *[_p(x) for x in out])
     if rc:
         raise RuntimeError("oracle_faces_from_potential rc=%d" % rc)
     return out

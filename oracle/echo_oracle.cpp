@@ -20,6 +20,12 @@
 //   edge array  E[k][c]   : point value of E_k at the k-edge displaced +1/2 in the two
 //                           directions (k+1)%3 and (k+2)%3 from the centre of cell c
 //
+// Scheme switches of the paper (oracle_set_scheme; defaults UCT=YES, HO=YES are the scheme of every test that
+// does not say otherwise): HO=NO makes INT and DER second order ("INT and DER ... only if higher than
+// second order accuracy is imposed (with the specific flag HO=YES)"); UCT=NO evolves a cell-centred B like the
+// other conserved variables, with no divergence control ("the magnetic field is not staggered but it is
+// treated as the other cell-centered variables").
+//
 // Pins (tests/test_oracle_*.py): see the list in DESIGN.md §"Oracle pins".
 // parity unpinned: the MP5 limiter branch on non-smooth data (the paper prints nothing
 // that fixes it; only its invariants are tested).
@@ -56,6 +62,9 @@ double der5(const double f[5]) {
     const double d0 = 1067.0 / 960.0, d2 = -29.0 / 480.0, d4 = 3.0 / 640.0;
     return d0 * f[2] + d2 * (f[1] + f[3]) + d4 * (f[0] + f[4]);
 }
+// HO switch: second-order INT = two-point average, second-order DER = identity
+double int_ho(const double b[6], int ho) { return ho ? int6(b) : 0.5 * (b[2] + b[3]); }
+double der_ho(const double f[5], int ho) { return ho ? der5(f) : f[2]; }
 
 // ----------------------------------------------------------------------------------
 // O3 — REC: MP5 (Suresh & Huynh 1997) on POINT values ("five elements ... MP5 ...
@@ -147,6 +156,13 @@ void phys_flux(double gam, const double q[8], int d, double F[5]) {
     F[4] = y * v[d] + ExB[d];
 }
 
+// UCT=NO: induction fluxes of the cell-centred B (eq.(8): dB/dt + curl E = 0, E = -v x B):
+// F_d(B_i) = v_d B_i - v_i B_d  (zero for i = d).
+void phys_flux_b(const double q[8], int d, double F[3]) {
+    const double *v = q + 1, *B = q + 5;
+    for (int a = 0; a < 3; ++a) F[a] = v[d] * B[a] - v[a] * B[d];
+}
+
 // O4 — fast characteristic speeds along d ("fast characteristic speeds"; S5):
 // lam[0] = lambda_+, lam[1] = lambda_-.
 void fast_speeds(double gam, const double q[8], int d, double lam[2]) {
@@ -169,7 +185,7 @@ void fast_speeds(double gam, const double q[8], int d, double lam[2]) {
 // O5 — two-state HLL flux at a d-face (S4).  qL, qR carry the SAME normal B_d.
 // F[5]; ex[4] = (a+, a-, vbar_{t1}, vbar_{t2}) with t1=(d+1)%3, t2=(d+2)%3 — the "fast
 // characteristic speeds and contributions for UCT" that P:L129 says are stored.
-void hll(double gam, const double qL[8], const double qR[8], int d, double F[5], double ex[4]) {
+void hll(double gam, const double qL[8], const double qR[8], int d, double F[5], double ex[4], double *FB = nullptr) {
     double lamL[2], lamR[2], FL[5], FR[5], UL[5], UR[5];
     fast_speeds(gam, qL, d, lamL);
     fast_speeds(gam, qR, d, lamR);
@@ -180,6 +196,12 @@ void hll(double gam, const double qL[8], const double qR[8], int d, double F[5],
     prim2cons(gam, qL, UL);
     prim2cons(gam, qR, UR);
     for (int c = 0; c < 5; ++c) F[c] = (ap * FL[c] + am * FR[c] - ap * am * (UR[c] - UL[c])) / (ap + am);
+    if (FB) {   // UCT=NO: the same two-state formula for the three cell-centred B components
+        double BL[3], BR[3];
+        phys_flux_b(qL, d, BL);
+        phys_flux_b(qR, d, BR);
+        for (int a = 0; a < 3; ++a) FB[a] = (ap * BL[a] + am * BR[a] - ap * am * (qR[5 + a] - qL[5 + a])) / (ap + am);
+    }
     const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
     ex[0] = ap;
     ex[1] = am;
@@ -275,7 +297,7 @@ struct Grid {
 
 struct State {
     Field U[5];   // D, Sx, Sy, Sz, U at cell centres
-    Field Bf[3];  // staggered B_d at d-faces
+    Field Bf[3];  // UCT=YES: staggered B_d at d-faces;  UCT=NO: the cell-centred B_d (evolved like U)
     void resize(long N) {
         for (auto &f : U) f.assign(N, 0.0);
         for (auto &f : Bf) f.assign(N, 0.0);
@@ -287,6 +309,7 @@ struct Stats { long calls = 0, fails = 0, sumit = 0; int maxit = 0; };
 struct Ctx {
     Grid g;
     double gam, cfl;
+    int uct = 1, ho = 1;   // scheme switches
     State s;
     bool has_state = false;
     double t = 0.0, dt_last = 0.0, amax = 0.0;
@@ -296,21 +319,22 @@ struct Ctx {
 };
 
 // Step 1 of a sub-step: INT of the staggered B to centres, then con2prim everywhere.
-void centre_b(const Grid &g, const Field Bf[3], Field Bc[3]) {
+void centre_b(const Grid &g, const Field Bf[3], Field Bc[3], int ho = 1) {
     for (int d = 0; d < 3; ++d) {
         Bc[d].assign(g.N, 0.0);
         FOR_CELLS(g, c) {
             CELL(c);
             double b[6];
             for (int m = 0; m < 6; ++m) b[m] = Bf[d][g.shift(c, d, m - 3)];  // faces i-5/2 .. i+5/2
-            Bc[d][g.idx(c[0], c[1], c[2])] = int6(b);
+            Bc[d][g.idx(c[0], c[1], c[2])] = int_ho(b, ho);
         }
     }
 }
 
 void primitives(const Ctx &cx, const State &s, Field P[5], Field Bc[3], Stats &st) {
     const Grid &g = cx.g;
-    centre_b(g, s.Bf, Bc);
+    if (cx.uct) centre_b(g, s.Bf, Bc, cx.ho);
+    else for (int d = 0; d < 3; ++d) Bc[d] = s.Bf[d];   // UCT=NO: the evolved field is already cell-centred
     for (int v = 0; v < 5; ++v) P[v].assign(g.N, 0.0);
     st = Stats();
     for (long c = 0; c < g.N; ++c) {
@@ -332,6 +356,7 @@ struct Rhs {
     Field B[3];
     Field E[3];      // edge EMFs (kept for tests)
     Field F[3][5];   // face fluxes per direction (kept for tests)
+    Field FB[3][3];  // UCT=NO: face fluxes of the three cell-centred B components, per direction
     double amax;
 };
 
@@ -349,6 +374,7 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
     for (int d = 0; d < 3; ++d) {
         const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
         for (int c = 0; c < 5; ++c) r.F[d][c].assign(g.N, 0.0);
+        for (int a = 0; a < 3; ++a) r.FB[d][a].assign(cx.uct ? 0 : g.N, 0.0);
         ap[d].assign(g.N, 0.0);
         am[d].assign(g.N, 0.0);
         vbar[d][0].assign(g.N, 0.0);
@@ -369,9 +395,19 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
                 qL[slot[v]] = mp5(sl);
                 qR[slot[v]] = mp5(sr);
             }
-            qL[5 + d] = qR[5 + d] = s.Bf[d][i0];  // the normal B is the staggered value itself
-            double F[5], ex[4];
-            hll(gam, qL, qR, d, F, ex);
+            double F[5], ex[4], FB[3];
+            if (cx.uct) {
+                qL[5 + d] = qR[5 + d] = s.Bf[d][i0];  // the normal B is the staggered value itself
+                hll(gam, qL, qR, d, F, ex);
+            } else {                                  // UCT=NO: the normal B is reconstructed like the rest
+                const Field &f = Bc[d];
+                const double sl[5] = {f[nb[0]], f[nb[1]], f[nb[2]], f[nb[3]], f[nb[4]]};
+                const double sr[5] = {f[nb[5]], f[nb[4]], f[nb[3]], f[nb[2]], f[nb[1]]};
+                qL[5 + d] = mp5(sl);
+                qR[5 + d] = mp5(sr);
+                hll(gam, qL, qR, d, F, ex, FB);
+                for (int a = 0; a < 3; ++a) r.FB[d][a][i0] = FB[a];
+            }
             for (int cc = 0; cc < 5; ++cc) r.F[d][cc][i0] = F[cc];
             ap[d][i0] = ex[0];
             am[d][i0] = ex[1];
@@ -384,22 +420,28 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
 
     // ---- point 3: DER + divergence, per direction; sources vanish (Minkowski)
     for (int c = 0; c < 5; ++c) r.U[c].assign(g.N, 0.0);
+    for (int a = 0; a < 3; ++a) r.B[a].assign(g.N, 0.0);
     for (int d = 0; d < 3; ++d) {
-        for (int cc = 0; cc < 5; ++cc) {
-            const Field &F = r.F[d][cc];
+        for (int cc = 0; cc < (cx.uct ? 5 : 8); ++cc) {
+            const Field &F = cc < 5 ? r.F[d][cc] : r.FB[d][cc - 5];
+            Field &out = cc < 5 ? r.U[cc] : r.B[cc - 5];
             Field Fh(g.N);
             FOR_CELLS(g, c) {
                 CELL(c);
                 double f[5];
                 for (int m = 0; m < 5; ++m) f[m] = F[g.shift(c, d, m - 2)];
-                Fh[g.idx(c[0], c[1], c[2])] = der5(f);
+                Fh[g.idx(c[0], c[1], c[2])] = der_ho(f, cx.ho);
             }
             FOR_CELLS(g, c) {
                 CELL(c);
                 const long i0 = g.idx(c[0], c[1], c[2]);
-                r.U[cc][i0] -= (Fh[i0] - Fh[g.shift(c, d, -1)]) / g.h[d];
+                out[i0] -= (Fh[i0] - Fh[g.shift(c, d, -1)]) / g.h[d];
             }
         }
+    }
+    if (!cx.uct) {   // UCT=NO: no edge EMFs, the rhs of the cell-centred B is the flux divergence above
+        for (int k = 0; k < 3; ++k) r.E[k].assign(g.N, 0.0);
+        return;
     }
 
     // ---- point 4: UCT edge EMFs with REC + upwind formula (O7)
@@ -443,9 +485,9 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
             CELL(c);
             double f[5];
             for (int m = 0; m < 5; ++m) f[m] = r.E[k][g.shift(c, j, m - 2)];
-            Ekh[g.idx(c[0], c[1], c[2])] = der5(f);
+            Ekh[g.idx(c[0], c[1], c[2])] = der_ho(f, cx.ho);
             for (int m = 0; m < 5; ++m) f[m] = r.E[j][g.shift(c, k, m - 2)];
-            Ejh[g.idx(c[0], c[1], c[2])] = der5(f);
+            Ejh[g.idx(c[0], c[1], c[2])] = der_ho(f, cx.ho);
         }
         r.B[i].assign(g.N, 0.0);
         FOR_CELLS(g, c) {
@@ -489,7 +531,7 @@ void rk3_step(Ctx &cx, double t_end) {
 }
 
 // S10 — the discrete divergence that UCT + DER preserves: sum_d D_d[DER_d B_d].
-void div_b(const Grid &g, const Field Bf[3], Field &div) {
+void div_b(const Grid &g, const Field Bf[3], Field &div, int ho = 1) {
     div.assign(g.N, 0.0);
     for (int d = 0; d < 3; ++d) {
         Field Bh(g.N);
@@ -497,7 +539,7 @@ void div_b(const Grid &g, const Field Bf[3], Field &div) {
             CELL(c);
             double f[5];
             for (int m = 0; m < 5; ++m) f[m] = Bf[d][g.shift(c, d, m - 2)];
-            Bh[g.idx(c[0], c[1], c[2])] = der5(f);
+            Bh[g.idx(c[0], c[1], c[2])] = der_ho(f, ho);
         }
         FOR_CELLS(g, c) {
             CELL(c);
@@ -509,7 +551,7 @@ void div_b(const Grid &g, const Field Bf[3], Field &div) {
 
 // S11 — staggered B from an edge-centred vector potential: the same discrete curl as O8
 // (B = +curl A), so that div_b of the result vanishes to round-off for any A.
-void curl_of_potential(const Grid &g, const double *const A[3], double *const B[3]) {
+void curl_of_potential(const Grid &g, const double *const A[3], double *const B[3], int ho = 1) {
     for (int i = 0; i < 3; ++i) {
         const int j = (i + 1) % 3, k = (i + 2) % 3;
         Field Akh(g.N), Ajh(g.N);
@@ -517,9 +559,9 @@ void curl_of_potential(const Grid &g, const double *const A[3], double *const B[
             CELL(c);
             double f[5];
             for (int m = 0; m < 5; ++m) f[m] = A[k][g.shift(c, j, m - 2)];
-            Akh[g.idx(c[0], c[1], c[2])] = der5(f);
+            Akh[g.idx(c[0], c[1], c[2])] = der_ho(f, ho);
             for (int m = 0; m < 5; ++m) f[m] = A[j][g.shift(c, k, m - 2)];
-            Ajh[g.idx(c[0], c[1], c[2])] = der5(f);
+            Ajh[g.idx(c[0], c[1], c[2])] = der_ho(f, ho);
         }
         FOR_CELLS(g, c) {
             CELL(c);
@@ -555,6 +597,30 @@ void *oracle_create(int nx, int ny, int nz, double gamma, double cfl) {
 
 void oracle_destroy(void *h) { delete static_cast<Ctx *>(h); }
 
+// Scheme switches of the paper; call before oracle_set_primitives.  With uct = 0 the three
+// "face" arrays of set/get_primitives are the CELL-CENTRED B.
+int oracle_set_scheme(void *h, int uct, int ho) {
+    Ctx *cx = static_cast<Ctx *>(h);
+    if (!cx || cx->has_state) return -4;
+    cx->uct = uct ? 1 : 0;
+    cx->ho = ho ? 1 : 0;
+    return 0;
+}
+
+// faces from an edge potential with the second-order (HO=NO) or sixth-order curl
+int oracle_faces_from_potential_ho(int nx, int ny, int nz, int ho, const double *ax, const double *ay, const double *az,
+                                   double *bx, double *by, double *bz) {
+    if (nx < 1 || ny < 1 || nz < 1) return -1;
+    Grid g;
+    g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+    for (int d = 0; d < 3; ++d) g.h[d] = 1.0 / g.n[d];
+    g.N = (long)nx * ny * nz;
+    const double *const A[3] = {ax, ay, az};
+    double *const B[3] = {bx, by, bz};
+    curl_of_potential(g, A, B, ho);
+    return 0;
+}
+
 // Cell-centred rho, v, p and face-staggered B point values -> conserved state; t = 0.
 int oracle_set_primitives(void *h, const double *rho, const double *vx, const double *vy, const double *vz,
                           const double *p, const double *bxf, const double *byf, const double *bzf) {
@@ -564,7 +630,8 @@ int oracle_set_primitives(void *h, const double *rho, const double *vx, const do
     const double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d) cx->s.Bf[d].assign(bf[d], bf[d] + g.N);
     Field Bc[3];
-    centre_b(g, cx->s.Bf, Bc);
+    if (cx->uct) centre_b(g, cx->s.Bf, Bc, cx->ho);
+    else for (int d = 0; d < 3; ++d) Bc[d] = cx->s.Bf[d];   // UCT=NO: the arrays given are cell-centred
     for (long c = 0; c < g.N; ++c) {
         const double q[8] = {rho[c], vx[c], vy[c], vz[c], p[c], Bc[0][c], Bc[1][c], Bc[2][c]};
         double u[5];
@@ -663,7 +730,7 @@ int oracle_div_b(void *h, double *div_field, double *max_abs) {
     Ctx *cx = static_cast<Ctx *>(h);
     if (!cx || !cx->has_state) return -4;
     Field div;
-    div_b(cx->g, cx->s.Bf, div);
+    div_b(cx->g, cx->s.Bf, div, cx->ho);
     double m = 0.0;
     for (long c = 0; c < cx->g.N; ++c) m = std::fmax(m, std::fabs(div[c]));
     if (div_field) std::memcpy(div_field, div.data(), sizeof(double) * cx->g.N);
@@ -692,7 +759,7 @@ int oracle_diagnostics(void *h, double out[24]) {
         out[9 + d] = (double)(sum * vol);
     }
     Field div;
-    div_b(g, cx->s.Bf, div);
+    div_b(g, cx->s.Bf, div, cx->ho);   // (UCT=NO: the same stencil applied to the cell-centred field; not preserved)
     double m = 0.0;
     for (long c = 0; c < g.N; ++c) m = std::fmax(m, std::fabs(div[c]));
     out[12] = m;
