@@ -44,6 +44,12 @@ typedef struct echo_ctx echo_ctx;
  * Courant number cfl > 0 (dt = cfl * min_d h_d / a_max, S9).  Returns NULL on bad arguments. */
 echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl);
 
+/* Host only.  The paper's scheme switches, to be called before echo_set_primitives.
+ * ho = 0: INT and DER second order (two-point average, identity) instead of sixth; everything else unchanged; the
+ * divergence UCT then preserves is the plain two-point one.  uct = 0 (cell-centred B, no divergence control) exists
+ * in the oracle only: ECHO_EINVAL here.  Defaults: uct = 1, ho = 1. */
+int echo_set_scheme(echo_ctx *ctx, int uct, int ho);
+
 /* Host only.  Frees the handle (never the workspace). */
 void echo_destroy(echo_ctx *ctx);
 

@@ -20,6 +20,7 @@ _vp, _dbl, _int, _long, _sz = C.c_void_p, C.c_double, C.c_int, C.c_long, C.c_siz
 SIGNATURES = {
     "echo_create": (_vp, [_int, _int, _int, _dbl, _dbl]),
     "echo_destroy": (None, [_vp]),
+    "echo_set_scheme": (_int, [_vp, _int, _int]),
     "echo_workspace_bytes": (_sz, [_vp]),
     "echo_bind": (_int, [_vp, _vp, _sz, _vp]),
     "echo_last_error": (C.c_char_p, [_vp]),
@@ -100,7 +101,7 @@ class EchoError(RuntimeError):
 class Echo:
     """One periodic unit box on the current CUDA device.  Tensors are torch.float64, shape (nz, ny, nx)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None):
+    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True):
         """block = (gnx, gny, gnz, halo_x, halo_y, halo_z): a domain-decomposition block (echo_create_block)."""
         torch = _torch()
         self.L = lib()
@@ -114,6 +115,8 @@ class Echo:
             self.h = self.L.echo_create_block(nx, ny, nz, gamma, cfl, *[int(b) for b in block])
         if not self.h:
             raise ValueError("echo_create: bad arguments")
+        if not ho:
+            self._check(self.L.echo_set_scheme(self.h, 1, 0))
         nbytes = self.L.echo_workspace_bytes(self.h)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned by the caller side
         self._check(self.L.echo_bind(self.h, self.workspace.data_ptr(), nbytes, _stream()))

@@ -123,7 +123,10 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
     const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
     const int C = (g.n[D] + nchunk - 1) / nchunk;
     dim3 grid((g.n[TD] + T - 1) / T, nchunk, g.n[OD]);
-    KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+    if (g.ho)
+        KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, true><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+    else
+        KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, false><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
     return ECHO_OK;
 }
 
@@ -233,6 +236,8 @@ echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl) {
     g.s[0] = 1; g.s[1] = nx; g.s[2] = nx * ny;
     g.N = (long long)nx * ny * nz;
     for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; g.lo[d] = 0; g.hi[d] = g.n[d]; }
+    g.ho = 1;
+    g.uct = 1;
     c->gamma = gamma;
     c->cfl = cfl;
     c->gg = gamma / (gamma - 1.0);
@@ -538,6 +543,15 @@ echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, in
     c->hmin = std::fmin(g.h[0], std::fmin(g.h[1], g.h[2]));
     c->block = true;
     return c;
+}
+
+int echo_set_scheme(echo_ctx *ctx, int uct, int ho) {
+    if (!ctx) return ECHO_EINVAL;
+    if (ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_scheme must precede echo_set_primitives");
+    if (!uct) return fail(ctx, ECHO_EINVAL, "UCT=NO is not built in the CUDA path (oracle only); DESIGN.md row f2");
+    ctx->g.uct = 1;
+    ctx->g.ho = ho ? 1 : 0;
+    return ECHO_OK;
 }
 
 size_t echo_field_offset(const echo_ctx *ctx, int field) {

@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl
             double b[6];
 #pragma unroll
             for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
-            B[d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
+            B[d] = int_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]);
         }
         double u[5] = {__ldg(st.U[0] + c), __ldg(st.U[1] + c), __ldg(st.U[2] + c), __ldg(st.U[3] + c),
                        __ldg(st.U[4] + c)};
@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
         double b[6];
 #pragma unroll
         for (int m = 0; m < 6; ++m) b[m] = __ldg(bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
-        q[5 + d] = int6(b[0], b[1], b[2], b[3], b[4], b[5]);
+        q[5 + d] = int_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]);
     }
     double u[5];
     prim2cons(gg, q, u);
@@ -178,7 +178,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // loaded BEFORE the face arithmetic of the round, so their latency is hidden behind it.
 struct FluxUpd { const double *base[5]; const double *cur[5]; double *out[5]; double c0, c1; };
 
-template <int D, int NT, int MODE>
+template <int D, int NT, int MODE, bool HO>
 __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
                                              int want_amax, FluxUpd up) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
 #pragma unroll
             for (int c = 0; c < 5; ++c) {
                 const double *F = Fb + c * FV;
-                const double r = rold[c] + mrh * der_diff(F[sl[0]], F[sl[1]], F[sl[2]], F[sl[3]], F[sl[4]], F[sl[5]]);
+                const double r = rold[c] + mrh * der_diff_ho(HO ? 1 : 0, F[sl[0]], F[sl[1]], F[sl[2]], F[sl[3]], F[sl[4]], F[sl[5]]);
                 if (MODE == 1) {
                     if (active) up.out[c][o2] = up.c0 * ubase[c] + up.c1 * (ucur[c] + dt * r);
                 } else {
@@ -391,8 +391,8 @@ __device__ __forceinline__ double curl_comp(const Grid &g, const double *const E
     double a[6], b[6];
 #pragma unroll
     for (int m = 0; m < 6; ++m) { a[m] = __ldg(E[K] + ix[J][m]); b[m] = __ldg(E[J] + ix[K][m]); }
-    return -(g.rh[J] * der_diff(a[0], a[1], a[2], a[3], a[4], a[5]) -
-             g.rh[K] * der_diff(b[0], b[1], b[2], b[3], b[4], b[5]));
+    return -(g.rh[J] * der_diff_ho(g.ho, a[0], a[1], a[2], a[3], a[4], a[5]) -
+             g.rh[K] * der_diff_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]));
 }
 
 template <bool WITH_U>
@@ -471,7 +471,7 @@ __global__ void __launch_bounds__(256) k_divb(Grid g, const double *B0, const do
             double f[6];
 #pragma unroll
             for (int m = 0; m < 6; ++m) f[m] = __ldg(B[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
-            v += g.rh[d] * der_diff(f[0], f[1], f[2], f[3], f[4], f[5]);
+            v += g.rh[d] * der_diff_ho(g.ho, f[0], f[1], f[2], f[3], f[4], f[5]);
         }
         if (div) div[c] = v;
         v = fabs(v);

@@ -23,6 +23,14 @@ __device__ __forceinline__ double der_diff(double f0, double f1, double f2, doub
     return (75.0 / 64.0) * (f3 - f2) + ((-25.0 / 384.0) * (f4 - f1) + (3.0 / 640.0) * (f5 - f0));
 }
 
+// HO switch: with ho = 0 INT is the two-point average and DER the identity (second order)
+__device__ __forceinline__ double int_ho(int ho, double b0, double b1, double b2, double b3, double b4, double b5) {
+    return ho ? int6(b0, b1, b2, b3, b4, b5) : 0.5 * (b2 + b3);
+}
+__device__ __forceinline__ double der_diff_ho(int ho, double f0, double f1, double f2, double f3, double f4, double f5) {
+    return ho ? der_diff(f0, f1, f2, f3, f4, f5) : f3 - f2;
+}
+
 // ---------------------------------------------------------------- fast FP64 helpers
 // min / max without the IEEE NaN bookkeeping of fmin/fmax (one DSETP + selects)
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }

@@ -14,6 +14,9 @@ struct Grid {
     // that the caller refreshes after every stage.  Global reductions (a_max, con2prim failures) only look at
     // the interior.  A plain periodic box has lo = 0, hi = n.
     int lo[3], hi[3];
+    // scheme switches of the paper (echo_set_scheme): ho = 0 makes INT and DER second order;
+    // uct = 0 evolves a cell-centred B like the other conserved variables
+    int ho, uct;
 };
 
 // Device control block (first bytes of the workspace).  Everything echo_step needs between

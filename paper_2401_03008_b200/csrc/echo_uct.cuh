@@ -267,12 +267,12 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const
             const double *pz_x = &sXE[ps][0][ty * UCT_XRW + tx], *py_x = pz_x + BU_XE;     // E_z, E_y along x
             const double *pz_y = &sYE[ps][0][ty * UCT_TX + tx], *px_y = pz_y + BU_YE;      // E_z, E_x along y
             constexpr int S = UCT_TX;
-            const double dxEz = der_diff(pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
-            const double dxEy = der_diff(py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
-            const double dyEz = der_diff(pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
-            const double dyEx = der_diff(px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
-            const double dzEy = der_diff(wy[0], wy[1], wy[2], wy[3], wy[4], wy[5]);
-            const double dzEx = der_diff(wx[0], wx[1], wx[2], wx[3], wx[4], wx[5]);
+            const double dxEz = der_diff_ho(g.ho, pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
+            const double dxEy = der_diff_ho(g.ho, py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
+            const double dyEz = der_diff_ho(g.ho, pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
+            const double dyEx = der_diff_ho(g.ho, px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
+            const double dzEy = der_diff_ho(g.ho, wy[0], wy[1], wy[2], wy[3], wy[4], wy[5]);
+            const double dzEx = der_diff_ho(g.ho, wx[0], wx[1], wx[2], wx[3], wx[4], wx[5]);
             double rb[3];
             rb[0] = -(g.rh[1] * dyEz - g.rh[2] * dzEy);
             rb[1] = -(g.rh[2] * dzEx - g.rh[0] * dxEz);

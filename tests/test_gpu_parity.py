@@ -324,3 +324,31 @@ def test_async_host_readback_two_streams(torch, eb, ob):
     b.synchronize()
     for x, y in zip(oa, ob_):
         assert torch.equal(x, y)
+
+
+@pytest.mark.parametrize("shape", [(40, 24, 20), (33, 1, 7)])
+def test_ho_no_variant(torch, eb, ob, shape):
+    """Row f2, HO=NO (second-order INT/DER): L(U) and 6 steps against the oracle run with the same switch,
+    and the two-point divergence stays at round-off."""
+    w = inputs.turbulence(None, shape=shape)
+    b = ob.faces_from_potential(w["ax"], w["ay"], w["az"], ho=False)
+    w["bxf"], w["byf"], w["bzf"] = [x + w["b0"][d] for d, x in enumerate(b)]
+    o = ob.Oracle(*shape, G, 0.3, ho=False)
+    o.set_primitives(*[w[k] for k in SETK])
+    e = eb.Echo(*shape, G, 0.3, ho=False)
+    bg = e.faces_from_potential(dev(torch, w["ax"]), dev(torch, w["ay"]), dev(torch, w["az"]), w["b0"])
+    for d, k in enumerate(("bxf", "byf", "bzf")):
+        assert absinf(bg[d].cpu().numpy(), w[k]) <= 1e-13
+    e.set_primitives(*[dev(torch, w[k]) for k in SETK])
+    rg, ro = e.rhs(), o.rhs()
+    for name in ("rhsU", "rhsB", "E"):
+        for c in range(len(ro[name])):
+            assert absinf(rg[name][c].cpu().numpy(), ro[name][c]) <= 1e-11 * max(1.0, np.abs(ro[name][c]).max()), (name, c)
+    e.step(6)
+    o.step(6)
+    compare_prims(e, o, tight=1e-11)
+    assert e.div_b() <= 1e-11 and e.div_b() == pytest.approx(o.div_b(), abs=1e-11)
+    with pytest.raises(eb.EchoError):
+        e._check(e.L.echo_set_scheme(e.h, 1, 1))          # too late: the state exists
+    h2 = eb.Echo(8, 8, 8, G, 0.3)
+    assert h2.L.echo_set_scheme(h2.h, 0, 1) == eb.ECHO_EINVAL   # UCT=NO: oracle only
