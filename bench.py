@@ -41,6 +41,17 @@ ALGO = {
 }
 FLOP_PER_CELL_UPDATE = 3 * sum(v["flop"] for v in ALGO.values())          # ~8.4e3
 BYTES_PER_CELL_UPDATE = 8 * 3 * sum(v["dbl"] for v in ALGO.values())      # 2784
+# UCT = NO (--scheme cc-ho / cc-lo, row f2): 8 cell fields, no UCT and no separate update kernel
+#   k_prim   8 in, 5 prims + 3 B copies out = 16; stage 2 also reads rhs (8) and writes U1, B1 (8)
+#   k_flux_x 8 in, 8 rhs out = 16;  k_flux_y + 8 rhs in = 24;  k_flux_z stage 1: 24, stages 2-3: + cur (8) + U^n (8) = 40
+# flop: + one more MP5 pair and the three induction fluxes per face (nominal 60)
+ALGO_CC = {
+    "k_prim":   {"flop": 268, "dbl": (16 + 32 + 16) / 3.0},
+    "k_flux_x": {"flop": 674, "dbl": 16},
+    "k_flux_y": {"flop": 674, "dbl": 24},
+    "k_flux_z": {"flop": 674 + 48 * 2 / 3.0, "dbl": (24 + 40 + 40) / 3.0},
+}
+SCHEMES = {"uct-ho": (True, True), "uct-lo": (True, False), "cc-ho": (False, True), "cc-lo": (False, False)}
 
 
 def measured_peaks():
@@ -174,6 +185,12 @@ def run_gpu(args):
 
     n, K, W = args.n, args.steps, max(args.warmup, 3)
     N = n ** 3
+    uct, ho = SCHEMES[args.scheme]
+    if args.scheme != "uct-ho" and (args.workload != "cpa" or args.decompose):
+        raise SystemExit("--scheme variants are wired for the default cpa workload only")
+    ALGO = globals()["ALGO"] if uct else ALGO_CC
+    FLOP_PER_CELL_UPDATE = 3 * sum(v["flop"] for v in ALGO.values())
+    BYTES_PER_CELL_UPDATE = 8 * 3 * sum(v["dbl"] for v in ALGO.values())
     decomposed = bool(args.decompose) and world > 1
     if decomposed:
         # ONE periodic box of (n px, n py, n pz) cells, one n^3 block (+ width-8 halos) per rank: halo exchange of
@@ -210,10 +227,11 @@ def run_gpu(args):
         parallelism = "replicas x%d (no collective)" % world
     else:
         w = inputs.cpa_wave(n, n, n, direction=args.direction)
-        e = binding.Echo(n, n, n, GAMMA, CFL)
+        e = binding.Echo(n, n, n, GAMMA, CFL, uct=uct, ho=ho)
         stepper = e.step
         parallelism = "replicas x%d (no collective)" % world
-    host = [torch.from_numpy(np.ascontiguousarray(w[k])).pin_memory() for k in SETK]
+    setk = SETK if uct else "rho vx vy vz p bx by bz".split()       # UCT = NO evolves the cell-centred B
+    host = [torch.from_numpy(np.ascontiguousarray(w[k])).pin_memory() for k in setk]
     devin = [h.to("cuda", non_blocking=True) for h in host]
     e.set_primitives(*devin)
     del devin
@@ -264,7 +282,7 @@ def run_gpu(args):
         # step (PCIe, both directions) overlap the kernels of the other; every step still moves all its bytes
         side = torch.cuda.Stream()
         with torch.cuda.stream(side):
-            e_b = binding.Echo(*e.n, GAMMA, CFL)
+            e_b = binding.Echo(*e.n, GAMMA, CFL, uct=uct, ho=ho)
         outs_b = [torch.empty(e.shape, dtype=torch.float64).pin_memory() for _ in range(8)]
         lanes = [(e, outs), (e_b, outs_b)]
         for h, o in lanes:
@@ -317,7 +335,7 @@ def run_gpu(args):
                 "frac": kd["tflops"] / fp64_sust}
     else:
         roof = {"bound": "hbm", "achieved": kd["gbs"], "peak": hbm_peak, "unit": "GB/s", "frac": kd["gbs"] / hbm_peak}
-    roof.update(kernel=dom, traffic=(TRAFFIC_PER_CELL[dom] * N if dom in TRAFFIC_PER_CELL else None),
+    roof.update(kernel=dom, traffic=(TRAFFIC_PER_CELL[dom] * N if dom in TRAFFIC_PER_CELL and args.scheme == "uct-ho" else None),
                 traffic_source="ncu dram bytes per cell of profiles/r1_ncu_full.md (256^3, stage 2) x cells of this launch", peak_source=("FP64 DFMA micro-benchmark run by this bench "
                 "(sustained; burst %.1f)" % fp64_burst) if roof["bound"] == "alu" else "MEASURED_PEAKS.json (%s)" % peak_kind,
                 algorithmic_flop_per_cell=ALGO[dom]["flop"], algorithmic_bytes_per_cell=8 * ALGO[dom]["dbl"],
@@ -338,7 +356,10 @@ def run_gpu(args):
             "config": {"workload": {"turb2d": "turbulence_2.5d_%d^2" % n, "turb3d": "alfvenic_turbulence_%d^3" % n}.get(
                            args.workload, "cpa_wave_%s_%d^3" % (args.direction, n)),
                        "grid": list(e.n), "gamma": GAMMA, "cfl": CFL,
-                       "scheme": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)", "cells": N,
+                       "scheme": {"uct-ho": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)",
+                                  "uct-lo": "MP5+HLL+UCT+SSPRK3, second-order INT/DER (UCT=YES, HO=NO)",
+                                  "cc-ho": "MP5+HLL+DER6+SSPRK3, cell-centred B (UCT=NO, HO=YES)",
+                                  "cc-lo": "MP5+HLL+SSPRK3, cell-centred B (UCT=HO=NO)"}[args.scheme], "cells": N,
                        "parallelism": parallelism,
                        "cache": "working set %.1f GB per GPU, far larger than the 126 MB L2" % (44 * 8 * N / 1e9)},
             "clocks": clocks,
@@ -384,6 +405,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--workload", default="cpa", choices=["cpa", "turb2d", "turb3d"],
                     help="cpa: BASELINE.json configs (default); turb2d: the paper's 2.5-D turbulence on n x n x 1")
+    ap.add_argument("--scheme", default="uct-ho", choices=sorted(SCHEMES),
+                    help="the paper's switches (P:L124, L138): uct-ho = UCT=HO=YES (default, the headline), "
+                         "uct-lo = HO=NO, cc-ho / cc-lo = UCT=NO with the cell-centred B (row f2)")
     ap.add_argument("--decompose", action="store_true",
                     help="N > 1: one decomposed box (n^3 cells per rank, halo exchange) instead of N replicas")
     args = ap.parse_args()

@@ -46,8 +46,13 @@ echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl);
 
 /* Host only.  The paper's scheme switches, to be called before echo_set_primitives.
  * ho = 0: INT and DER second order (two-point average, identity) instead of sixth; everything else unchanged; the
- * divergence UCT then preserves is the plain two-point one.  uct = 0 (cell-centred B, no divergence control) exists
- * in the oracle only: ECHO_EINVAL here.  Defaults: uct = 1, ho = 1. */
+ * divergence UCT then preserves is the plain two-point one.  uct = 0: the cell-centred B is evolved by flux
+ * differences like the other conserved variables, with no divergence control; the three "face" arrays of
+ * echo_set_primitives[_host] / echo_get_primitives[_host] then hold (and return) the CELL-CENTRED B, echo_rhs returns
+ * the rhs of that B in rhsB and zeros in E, echo_div_b applies its face formula to those arrays (not a conserved
+ * quantity of this scheme).  uct = 0 on a block handle (echo_create_block): ECHO_EINVAL, and echo_stage_sweeps /
+ * echo_stage_finish return ECHO_EINVAL on a uct = 0 handle.  ECHO_ESTATE once a state exists.
+ * Defaults: uct = 1, ho = 1. */
 int echo_set_scheme(echo_ctx *ctx, int uct, int ho);
 
 /* Host only.  Frees the handle (never the workspace). */

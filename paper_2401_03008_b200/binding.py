@@ -101,8 +101,10 @@ class EchoError(RuntimeError):
 class Echo:
     """One periodic unit box on the current CUDA device.  Tensors are torch.float64, shape (nz, ny, nx)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True):
-        """block = (gnx, gny, gnz, halo_x, halo_y, halo_z): a domain-decomposition block (echo_create_block)."""
+    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True, uct=True):
+        """block = (gnx, gny, gnz, halo_x, halo_y, halo_z): a domain-decomposition block (echo_create_block).
+        ho / uct: the paper's scheme switches (echo_set_scheme); with uct=False the three "face" arrays of
+        set_primitives / get_primitives are the cell-centred B."""
         torch = _torch()
         self.L = lib()
         self.n = (nx, ny, nz)
@@ -115,8 +117,8 @@ class Echo:
             self.h = self.L.echo_create_block(nx, ny, nz, gamma, cfl, *[int(b) for b in block])
         if not self.h:
             raise ValueError("echo_create: bad arguments")
-        if not ho:
-            self._check(self.L.echo_set_scheme(self.h, 1, 0))
+        if not (ho and uct):
+            self._check(self.L.echo_set_scheme(self.h, int(bool(uct)), int(bool(ho))))
         nbytes = self.L.echo_workspace_bytes(self.h)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned by the caller side
         self._check(self.L.echo_bind(self.h, self.workspace.data_ptr(), nbytes, _stream()))

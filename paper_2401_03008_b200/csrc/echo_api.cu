@@ -115,14 +115,32 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
     if (g.n[D] == 1) {   // a one-cell axis: no stencil work left, only the face quantities (k_flux_flat)
-        KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
-               g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        if (g.uct)
+            KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
+                   g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        else
+            KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
+                   g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
         return ECHO_OK;
     }
     // chunks along D: one chunk per column unless the axis is long (5 halo faces per chunk are recomputed)
     const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
     const int C = (g.n[D] + nchunk - 1) / nchunk;
     dim3 grid((g.n[TD] + T - 1) / T, nchunk, g.n[OD]);
+    if (!g.uct) {   // UCT = NO: 8 flux components, rings of 49 KB in dynamic shared memory
+        constexpr int R = NT / T, RL = 3 * R, SB = RL + 4;   // as in k_flux
+        constexpr size_t smem = sizeof(double) * ((D == 0) ? (8 + 8) * T * SB : RL * (8 + 8) * T);
+        if (g.ho) {
+            auto kern = k_flux<D, NT, MODE, true, false>;
+            CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            KL(KC_FLUX + D, "k_flux_cc", kern<<<grid, NT, smem, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        } else {
+            auto kern = k_flux<D, NT, MODE, false, false>;
+            CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            KL(KC_FLUX + D, "k_flux_cc", kern<<<grid, NT, smem, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        }
+        return ECHO_OK;
+    }
     if (g.ho)
         KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, true><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
     else
@@ -142,13 +160,19 @@ struct StagePlan {
 int launch_sweeps(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan *pl = nullptr) {
     const Grid &g = ctx->g;
     PrimUpd pu;
-    for (int v = 0; v < 5; ++v) pu.uout[v] = ctx->field[F_U1 + v];
-    if (pl && pl->prim_upd)
+    for (int v = 0; v < 8; ++v) pu.uout[v] = ctx->field[F_U1 + v];
+    for (int d = 0; d < 3; ++d) pu.bin[d] = ctx->field[F_BF + d];
+    if (!g.uct) {
+        if (pl && pl->prim_upd)
+            KL(KC_PRIM, "k_prim_cc", k_prim<false, true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+        else
+            KL(KC_PRIM, "k_prim_cc", k_prim<false, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+    } else if (pl && pl->prim_upd)
         KL(KC_PRIM, "k_prim", k_prim<false, true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
     else
         KL(KC_PRIM, "k_prim", k_prim<false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
     FluxUpd fu;
-    for (int v = 0; v < 5; ++v) {
+    for (int v = 0; v < 8; ++v) {
         fu.base[v] = ctx->field[F_U + v];
         fu.cur[v] = ctx->field[((pl && pl->cur) ? F_U1 : F_U) + v];
         fu.out[v] = ctx->field[((pl && pl->out) ? F_U1 : F_U) + v];
@@ -186,6 +210,10 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
 int launch_operator(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan *pl = nullptr) {
     int rc;
     if ((rc = launch_sweeps(ctx, st, want_amax, pl))) return rc;
+    if (!ctx->g.uct) {   // UCT = NO: the sweeps already hold the rhs of B; only dt is left (stage 1)
+        if (want_amax == 2) KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
+        return ECHO_OK;
+    }
     return launch_uct(ctx, st, want_amax == 2);
 }
 
@@ -328,6 +356,22 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     if (rc) return rc;
     if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    if (!ctx->g.uct) {
+        // UCT = NO: all 8 fields are cell fields.  Stage 1 writes rhs only; its update is formed by the
+        // k_prim of stage 2 (U and B); stages 2 and 3 combine all 8 fields inside their z-sweep.  10 launches.
+        for (int n = 0; n < nsteps; ++n) {
+            KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+            if ((rc = launch_operator(ctx, s0, 2))) return rc;
+            Stage s12 = s1;
+            for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];
+            const StagePlan p2 = {true, true, 1, 1, 0.75, 0.25};
+            if ((rc = launch_operator(ctx, s12, 0, &p2))) return rc;
+            const StagePlan p3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
+            if ((rc = launch_operator(ctx, s1, 0, &p3))) return rc;
+            KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+        }
+        return ECHO_OK;
+    }
     for (int n = 0; n < nsteps; ++n) {
         KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
         // stage 1: L(U^n), dt from its speeds (S9); B1 = B^n + dt rhs_B now, U1 = U^n + dt rhs_U deferred
@@ -363,7 +407,8 @@ int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, doub
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 5; ++v) st.P[v] = out[v];
     for (int d = 0; d < 3; ++d) st.Bc[d] = out[5 + d];
-    KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
     double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d)
         if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -379,7 +424,8 @@ static int get_primitives_host_impl(echo_ctx *ctx, double *rho, double *vx, doub
     const Grid &g = ctx->g;
     const size_t nb = sizeof(double) * g.N;
     Stage st = make_stage(ctx, 0);
-    KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 8; ++v) CU(cudaMemcpyAsync(out[v], ctx->field[F_P + v], nb, cudaMemcpyDeviceToHost, ctx->stream));
     double *bf[3] = {bxf, byf, bzf};
@@ -427,9 +473,13 @@ int echo_rhs(echo_ctx *ctx, double *const *rhsU, double *const *rhsB, double *co
     if ((rc = launch_operator(ctx, st, 1))) return rc;
     if (rhsU)
         for (int v = 0; v < 5; ++v) CU(cudaMemcpyAsync(rhsU[v], st.R[v], nb, cudaMemcpyDeviceToDevice, ctx->stream));
-    if (E)
+    if (E && !g.uct)
+        for (int d = 0; d < 3; ++d) CU(cudaMemsetAsync(E[d], 0, nb, ctx->stream));
+    else if (E)
         for (int d = 0; d < 3; ++d) CU(cudaMemcpyAsync(E[d], st.E[d], nb, cudaMemcpyDeviceToDevice, ctx->stream));
-    if (rhsB) {
+    if (rhsB && !g.uct) {   // UCT = NO: the sweeps left the rhs of the cell-centred B in the E fields; no EMFs
+        for (int d = 0; d < 3; ++d) CU(cudaMemcpyAsync(rhsB[d], st.E[d], nb, cudaMemcpyDeviceToDevice, ctx->stream));
+    } else if (rhsB) {
         KL(KC_OTHER, "k_curl", k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], rhsB[0], rhsB[1], rhsB[2],
                                                                1.0, 0.0, 0.0, 0.0));
     }
@@ -493,7 +543,8 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
                                            f + 7 * np, ctx->part));
     Stage st = make_stage(ctx, 0);
     KL(KC_CTRL, "k_c2p_stats_reset", k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
-    KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
     KL(KC_OTHER, "k_extrema", k_extrema<<<NPART, 256, 0, ctx->stream>>>(g.N, st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], ctx->part));
     double dmax = 0.0;
     if ((rc = echo_div_b(ctx, nullptr, &dmax))) return rc;   // synchronises
@@ -548,8 +599,8 @@ echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, in
 int echo_set_scheme(echo_ctx *ctx, int uct, int ho) {
     if (!ctx) return ECHO_EINVAL;
     if (ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_scheme must precede echo_set_primitives");
-    if (!uct) return fail(ctx, ECHO_EINVAL, "UCT=NO is not built in the CUDA path (oracle only); DESIGN.md row f2");
-    ctx->g.uct = 1;
+    if (!uct && ctx->block) return fail(ctx, ECHO_EINVAL, "UCT=NO is not built for block handles (echo_create_block)");
+    ctx->g.uct = uct ? 1 : 0;
     ctx->g.ho = ho ? 1 : 0;
     return ECHO_OK;
 }
@@ -573,6 +624,7 @@ int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
+    if (!ctx->g.uct) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES only");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     if (stage == 1) {
         KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
@@ -587,6 +639,7 @@ int echo_stage_finish(echo_ctx *ctx, int stage) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
+    if (!ctx->g.uct) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES only");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     if (stage == 1) {
         // dt from the (all-reduced) a_max, UCT, then the UNFUSED update of all 8 fields: U1 must exist in

@@ -60,9 +60,11 @@ __global__ void k_c2p_stats_reset(Ctrl *c) {
 // here, on the fly, by the INT+con2prim pass of stage 2 (st.U = U^n, st.R = L(U^n), result stored to
 // uout and inverted at once): dt only exists after all three stage-1 sweeps, and this kernel has
 // spare memory bandwidth, so the update costs no pass of its own and U1 is never re-read.
-struct PrimUpd { double *uout[5]; };
+// UCT = false: B is a cell-centred evolved field (st.Bf holds it); no INT, and the deferred update covers B too
+// (bin = B^n, rhs of B in st.E, result to uout[5..7]).
+struct PrimUpd { double *uout[8]; const double *bin[3]; };
 
-template <bool STATS, bool UPD>
+template <bool STATS, bool UPD, bool UCT = true>
 __global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -75,11 +77,18 @@ __global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl
         double B[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            const int base = c - g.s[d] * c3[d];
-            double b[6];
+            if (UCT) {
+                const int base = c - g.s[d] * c3[d];
+                double b[6];
 #pragma unroll
-            for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
-            B[d] = int_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]);
+                for (int m = 0; m < 6; ++m) b[m] = __ldg(st.Bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
+                B[d] = int_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]);
+            } else if (UPD) {
+                B[d] = __ldg(pu.bin[d] + c) + ctrl->dt * __ldg(st.E[d] + c);
+                pu.uout[5 + d][c] = B[d];
+            } else {
+                B[d] = __ldg(st.Bf[d] + c);
+            }
         }
         double u[5] = {__ldg(st.U[0] + c), __ldg(st.U[1] + c), __ldg(st.U[2] + c), __ldg(st.U[3] + c),
                        __ldg(st.U[4] + c)};
@@ -127,6 +136,7 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
                                               const double *vz, const double *p, const double *bf0,
                                               const double *bf1, const double *bf2, double *U0, double *U1,
                                               double *U2, double *U3, double *U4, double gg) {
+    // UCT = false: bf0..2 ARE the cell-centred B (no INT)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
@@ -141,7 +151,7 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
         double b[6];
 #pragma unroll
         for (int m = 0; m < 6; ++m) b[m] = __ldg(bf[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
-        q[5 + d] = int_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]);
+        q[5 + d] = g.uct ? int_ho(g.ho, b[0], b[1], b[2], b[3], b[4], b[5]) : b[3];
     }
     double u[5];
     prim2cons(gg, q, u);
@@ -176,9 +186,13 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // out = c0*base + c1*(cur + dt*rhs) (O9), so rhs is neither written nor re-read and the update
 // traffic rides under the arithmetic of the sweep.  The old rhs / state values a cell needs are
 // loaded BEFORE the face arithmetic of the round, so their latency is hidden behind it.
-struct FluxUpd { const double *base[5]; const double *cur[5]; double *out[5]; double c0, c1; };
+struct FluxUpd { const double *base[8]; const double *cur[8]; double *out[8]; double c0, c1; };   // 5 used with UCT
 
-template <int D, int NT, int MODE, bool HO>
+// UCT = false: the cell-centred B is reconstructed (all three components) and advanced by flux differences
+// like the other conserved variables: 8 reconstructed fields, 8 flux components (rhs of B in st.E), no face
+// quantities for UCT.  The inputs are the k_prim copies st.Bc, not the evolved st.Bf: the fused RK update of
+// MODE 1 overwrites the evolved B while wrapped rows of it are still to be read.  Compile-time branches only: the UCT = true instantiations are the kernel described above.
+template <int D, int NT, int MODE, bool HO, bool UCT = true>
 __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
                                              int want_amax, FluxUpd up) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
@@ -192,10 +206,15 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
     constexpr int SB = (D == 0) ? RL + 4 : 1;
     constexpr int SR = (D == 0) ? 1 : 8 * T;
     constexpr int SV = (D == 0) ? T * SB : T;
-    constexpr int FR = (D == 0) ? 1 : 5 * T;
+    constexpr int NC = UCT ? 5 : 8;           // flux components
+    constexpr int FR = (D == 0) ? 1 : NC * T;
     constexpr int FV = SV;
-    __shared__ double sP[(D == 0) ? 8 * T * SB : RL * 8 * T];
-    __shared__ double sF[(D == 0) ? 5 * T * SB : RL * 5 * T];
+    constexpr int PSZ = (D == 0) ? 8 * T * SB : RL * 8 * T, FSZ = (D == 0) ? NC * T * SB : RL * NC * T;
+    __shared__ double sPs[UCT ? PSZ : 1];
+    __shared__ double sFs[UCT ? FSZ : 1];
+    extern __shared__ double sdyn[];          // UCT = false needs 49 KB: dynamic shared memory
+    double *const sP = UCT ? sPs : sdyn;
+    double *const sF = UCT ? sFs : sdyn + PSZ;
 
     const int nD = g.n[D], nT = g.n[TD];
     const int m0 = blockIdx.y * C;
@@ -209,7 +228,8 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
     const int la = (D == 0) ? tid % R : tid / T;
     const int lb = (D == 0) ? tid / R : tid % T;
     const int lsrc = baseO + sT * min(t0 + lb, nT - 1);
-    const double *fld[8] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2], st.Bf[D]};
+    const double *fld[8] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], UCT ? st.Bc[t1] : st.Bc[0],
+                            UCT ? st.Bc[t2] : st.Bc[1], UCT ? st.Bf[D] : st.Bc[2]};
     auto issue = [&](int grp) {
         const int src = lsrc + sD * wrapi(m0 - 5 + R * grp + la, nD);
         double *dst = sP + ((grp % 3) * R + la) * SR + lb * SB;
@@ -240,15 +260,17 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
         const int i2 = R * (t - 1) - 5 + a;               // cell row within the chunk
         const bool do2 = (t >= 1) && colok && i2 >= 0 && i2 < Cv;
         const int o2 = ocol + sD * (m0 + i2);
-        double rold[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, ucur[5], ubase[5];
+        double rold[NC], ucur[NC], ubase[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) rold[c] = 0.0;
         if (do2) {
             if (D != 0) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) rold[c] = __ldg(st.R[c] + o2);
+                for (int c = 0; c < NC; ++c) rold[c] = __ldg((c < 5 ? st.R[c] : st.E[c - 5]) + o2);
             }
             if (MODE == 1) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) { ucur[c] = __ldg(up.cur[c] + o2); ubase[c] = __ldg(up.base[c] + o2); }
+                for (int c = 0; c < NC; ++c) { ucur[c] = __ldg(up.cur[c] + o2); ubase[c] = __ldg(up.base[c] + o2); }
             }
         }
 
@@ -262,25 +284,31 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
             for (int k = 0; k < 6; ++k) { sl[k] = r0 * SR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
             const double *Pb = sP + b * SB;
             double qL[8], qR[8];
-            constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+            constexpr int slot[8] = {0, 1, 2, 3, 4, UCT ? 5 + t1 : 5, UCT ? 5 + t2 : 6, 7};
 #pragma unroll
-            for (int v = 0; v < 7; ++v) {
+            for (int v = 0; v < (UCT ? 7 : 8); ++v) {
                 const double *p = Pb + v * SV;
                 const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
                 mp5_pair<true>(s0, s1, s2, s3, s4, s5, qL[slot[v]], qR[slot[v]]);
             }
-            qL[5 + D] = qR[5 + D] = Pb[7 * SV + sl[2]];   // the normal B is the staggered value
-            double F[5], ap, am, vb1, vb2;
-            hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
+            double F[NC], ap, am, vb1 = 0.0, vb2 = 0.0;
+            if (UCT) {
+                qL[5 + D] = qR[5 + D] = Pb[7 * SV + sl[2]];   // the normal B is the staggered value
+                hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
+            } else {
+                hll_face_cc<D>(gam, gg, qL, qR, F, ap, am);
+            }
             double *Fo = sF + b * SB + fslot;
 #pragma unroll
-            for (int c = 0; c < 5; ++c) Fo[c * FV] = F[c];
+            for (int c = 0; c < NC; ++c) Fo[c * FV] = F[c];
             if (f >= 3 && f < Cv + 3) {
                 const int o = ocol + sD * (m0 + f - 3);
-                st.ap[D][o] = ap;
-                st.am[D][o] = am;
-                st.vb[D][0][o] = vb1;
-                st.vb[D][1][o] = vb2;
+                if (UCT) {
+                    st.ap[D][o] = ap;
+                    st.am[D][o] = am;
+                    st.vb[D][0][o] = vb1;
+                    st.vb[D][1][o] = vb2;
+                }
                 const int cD = m0 + f - 3, cTT = t0 + b, cOO = (int)blockIdx.z;
                 const bool inner = cD >= g.lo[D] && cD < g.hi[D] && cTT >= g.lo[TD] && cTT < g.hi[TD] &&
                                    cOO >= g.lo[OD] && cOO < g.hi[OD];
@@ -297,13 +325,13 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
             for (int k = 0; k < 6; ++k) { sl[k] = r0 * FR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
             const double *Fb = sF + b * SB;
 #pragma unroll
-            for (int c = 0; c < 5; ++c) {
+            for (int c = 0; c < NC; ++c) {
                 const double *F = Fb + c * FV;
                 const double r = rold[c] + mrh * der_diff_ho(HO ? 1 : 0, F[sl[0]], F[sl[1]], F[sl[2]], F[sl[3]], F[sl[4]], F[sl[5]]);
                 if (MODE == 1) {
                     if (active) up.out[c][o2] = up.c0 * ubase[c] + up.c1 * (ucur[c] + dt * r);
                 } else {
-                    st.R[c][o2] = r;
+                    (c < 5 ? st.R[c] : st.E[c - 5])[o2] = r;
                 }
             }
         }
@@ -329,7 +357,7 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
 // face quantities UCT needs (a+, a-, vbar), a_max and, in MODE 1, the RK combination remain.  The arithmetic of
 // the face is the generic one applied to six equal stencil values, so a flat run stays bit-identical to the same
 // data on a thicker grid (dimensional-reduction test).
-template <int D, int MODE>
+template <int D, int MODE, bool UCT = true>
 __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam, double gg, Ctrl *ctrl, int want_amax,
                                                    FluxUpd up) {
     constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
@@ -339,33 +367,40 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
     double amax = 0.0;
     if (i < g.n[0] && j < g.n[1]) {
         const int c = i + g.s[1] * j + g.s[2] * k;
-        const double *rec[7] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], st.Bc[t1], st.Bc[t2]};
-        constexpr int slot[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+        constexpr int NC = UCT ? 5 : 8;
+        const double *rec[8] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], UCT ? st.Bc[t1] : st.Bc[0],
+                                UCT ? st.Bc[t2] : st.Bc[1], st.Bc[2]};
+        constexpr int slot[8] = {0, 1, 2, 3, 4, UCT ? 5 + t1 : 5, UCT ? 5 + t2 : 6, 7};
         double qL[8], qR[8];
 #pragma unroll
-        for (int v = 0; v < 7; ++v) {
+        for (int v = 0; v < (UCT ? 7 : 8); ++v) {
             const double s = __ldg(rec[v] + c);
             mp5_pair<true>(s, s, s, s, s, s, qL[slot[v]], qR[slot[v]]);
         }
-        qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + c);
-        double F[5], ap, am, vb1, vb2;
-        hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
-        st.ap[D][c] = ap;
-        st.am[D][c] = am;
-        st.vb[D][0][c] = vb1;
-        st.vb[D][1][c] = vb2;
+        double F[NC], ap, am, vb1, vb2;
+        if (UCT) {
+            qL[5 + D] = qR[5 + D] = __ldg(st.Bf[D] + c);
+            hll_face<D>(gam, gg, qL, qR, F, ap, am, vb1, vb2);
+            st.ap[D][c] = ap;
+            st.am[D][c] = am;
+            st.vb[D][0][c] = vb1;
+            st.vb[D][1][c] = vb2;
+        } else {
+            hll_face_cc<D>(gam, gg, qL, qR, F, ap, am);
+        }
         const bool inner = i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2];
         if (inner) amax = dmax(ap, am);
         if (MODE == 1) {
             const double dt = ctrl->dt;
             if (ctrl->active) {
 #pragma unroll
-                for (int v = 0; v < 5; ++v)
-                    up.out[v][c] = up.c0 * __ldg(up.base[v] + c) + up.c1 * (up.cur[v][c] + dt * __ldg(st.R[v] + c));
+                for (int v = 0; v < NC; ++v)
+                    up.out[v][c] = up.c0 * __ldg(up.base[v] + c) +
+                                   up.c1 * (up.cur[v][c] + dt * __ldg((v < 5 ? st.R[v] : st.E[v - 5]) + c));
             }
         } else if (D == 0) {
 #pragma unroll
-            for (int v = 0; v < 5; ++v) st.R[v][c] = 0.0;     // the x-sweep is the one that initialises rhs
+            for (int v = 0; v < NC; ++v) (v < 5 ? st.R[v] : st.E[v - 5])[c] = 0.0;   // the x-sweep initialises rhs
         }
     }
     if (want_amax) {

@@ -253,6 +253,29 @@ __device__ __forceinline__ void hll_face(double gam, double gg, const double qL[
     vb2 = wl * qL[1 + t2] + wr * qR[1 + t2];
 }
 
+// UCT=NO: the cell-centred B is a conserved variable like the others.  Same two-state formula as O5 for
+// 8 components; the induction fluxes are F_D(B_a) = v_D B_a - v_a B_D (eq.(8), with E = -v x B).  Both
+// sides carry their own reconstructed normal B.
+template <int D>
+__device__ __forceinline__ void hll_face_cc(double gam, double gg, const double qL[8], const double qR[8], double F[8],
+                                            double &ap, double &am) {
+    double uL[5], fL[5], uR[5], fR[5], lpL, lmL, lpR, lmR;
+    side_state<D>(gam, gg, qL, uL, fL, lpL, lmL);
+    side_state<D>(gam, gg, qR, uR, fR, lpR, lmR);
+    ap = dmax(0.0, dmax(lpL, lpR));
+    am = dmax(0.0, dmax(-lmL, -lmR));
+    const double inv = rcp_fast(ap + am);
+    const double wl = ap * inv, wr = am * inv, wd = ap * am * inv;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) F[c] = wl * fL[c] + wr * fR[c] - wd * (uR[c] - uL[c]);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double bL = qL[1 + D] * qL[5 + a] - qL[1 + a] * qL[5 + D];
+        const double bR = qR[1 + D] * qR[5 + a] - qR[1 + a] * qR[5 + D];
+        F[5 + a] = wl * bL + wr * bR - wd * (qR[5 + a] - qL[5 + a]);
+    }
+}
+
 // ---------------------------------------------------------------- O2: con2prim
 // Newton on y = rho h W^2 from the upper bound y0 = gamma (U - B^2/2); safeguard and stopping
 // rule as in DESIGN.md O2.  Returns the number of Newton updates (>=1) or -(count) on failure.

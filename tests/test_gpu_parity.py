@@ -350,5 +350,39 @@ def test_ho_no_variant(torch, eb, ob, shape):
     assert e.div_b() <= 1e-11 and e.div_b() == pytest.approx(o.div_b(), abs=1e-11)
     with pytest.raises(eb.EchoError):
         e._check(e.L.echo_set_scheme(e.h, 1, 1))          # too late: the state exists
-    h2 = eb.Echo(8, 8, 8, G, 0.3)
-    assert h2.L.echo_set_scheme(h2.h, 0, 1) == eb.ECHO_EINVAL   # UCT=NO: oracle only
+
+
+@pytest.mark.parametrize("shape,ho", [((40, 24, 20), True), ((40, 24, 20), False), ((33, 1, 7), True), ((19, 21, 1), False)])
+def test_uct_no_variant(torch, eb, ob, shape, ho):
+    """Row f2, UCT=NO (P:L124: the cell-centred B advanced by flux differences like the other conserved variables;
+    with HO=NO the configuration of the paper's best throughput): L(U) and 6 steps against the oracle run
+    with the same switches.  The three B arrays are cell-centred on both sides."""
+    w = inputs.turbulence(None, shape=shape)
+    nx, ny, nz = shape
+    z, y, x = np.meshgrid((np.arange(nz) + 0.5) / nz, (np.arange(ny) + 0.5) / ny, (np.arange(nx) + 0.5) / nx, indexing="ij")
+    bsm = ob.faces_from_potential(w["ax"], w["ay"], w["az"])
+    # the smooth turbulent field taken as cell values, plus a mode with div B != 0: nothing constrains it here
+    bcc = [bsm[d] + w["b0"][d] + 0.05 * np.cos(2 * np.pi * (x + 2 * y + 3 * z) + d) for d in range(3)]
+    args = [w[k] for k in ("rho", "vx", "vy", "vz", "p")] + bcc
+    o = ob.Oracle(*shape, G, 0.3, uct=False, ho=ho)
+    o.set_primitives(*args)
+    e = eb.Echo(*shape, G, 0.3, uct=False, ho=ho)
+    e.set_primitives(*[dev(torch, a) for a in args])
+    rg, ro = e.rhs(), o.rhs()
+    for name in ("rhsU", "rhsB"):
+        for c in range(len(ro[name])):
+            assert absinf(rg[name][c].cpu().numpy(), ro[name][c]) <= 1e-11 * max(1.0, np.abs(ro[name][c]).max()), (name, c)
+    assert rg["amax"] == pytest.approx(ro["amax"], rel=1e-13)
+    for c in range(3):
+        assert not rg["E"][c].any() and not ro["E"][c].any()      # no edge EMFs in this scheme
+    e.step(6)
+    o.step(6)
+    compare_prims(e, o, tight=1e-11)
+    dg, do = e.diagnostics(), o.diagnostics()
+    assert dg["t"] == pytest.approx(do["t"], rel=1e-13) and dg["c2p_failures"] == 0
+    for k in ("sum_D", "sum_U", "sum_Bx", "sum_By", "sum_Bz"):
+        assert dg[k] == pytest.approx(do[k], rel=1e-12, abs=1e-13), k
+    blk = eb.Echo(24, 8, 8, G, 0.3, block=(16, 8, 8, 8, 0, 0))
+    assert blk.L.echo_set_scheme(blk.h, 0, 1) == eb.ECHO_EINVAL   # block handles: UCT=YES only
+    with pytest.raises(eb.EchoError):
+        e.stage_sweeps(1)
