@@ -40,6 +40,9 @@ def lib():
         L.oracle_destroy.argtypes = [C.c_void_p]
         L.oracle_destroy.restype = None
         L.oracle_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.oracle_set_order.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.oracle_tvd2.restype = C.c_double
+        L.oracle_tvd2.argtypes = [_dp]
         L.oracle_faces_from_potential_ho.argtypes = [C.c_int] * 4 + [_dp] * 6
         L.oracle_set_primitives.argtypes = [C.c_void_p] + [_dp] * 8
         L.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
@@ -84,9 +87,10 @@ DIAG_NAMES = ["t", "dt_last", "steps", "amax", "sum_D", "sum_Sx", "sum_Sy", "sum
 class Oracle:
     """One periodic unit box.  Arrays are numpy float64 of shape (nz, ny, nx) (x fastest)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, uct=True, ho=True):
+    def __init__(self, nx, ny, nz, gamma, cfl, uct=True, ho=True, rec=5, rk=3):
         """uct / ho: the paper's scheme switches.  With uct=False the three B arrays given to
-        set_primitives (and returned as bxf, byf, bzf) are CELL-CENTRED."""
+        set_primitives (and returned as bxf, byf, bzf) are CELL-CENTRED.  rec / rk: 5 / 3 = MP5 + SSP-RK3 (default),
+        2 / 2 = limited linear reconstruction + SSP-RK2."""
         self.L = lib()
         self.shape = (nz, ny, nx)
         self.n = (nx, ny, nz)
@@ -95,6 +99,9 @@ class Oracle:
             raise ValueError("oracle_create: bad arguments")
         if not (uct and ho):
             rc = self.L.oracle_set_scheme(self.h, int(bool(uct)), int(bool(ho)))
+            assert rc == 0, rc
+        if (rec, rk) != (5, 3):
+            rc = self.L.oracle_set_order(self.h, int(rec), int(rk))
             assert rc == 0, rc
 
     def __del__(self):
@@ -206,6 +213,11 @@ def der5(f):
 def mp5(v):
     v = _c(v); assert v.size == 5
     return lib().oracle_mp5(_p(v))
+
+
+def tvd2(v):
+    v = _c(v); assert v.size == 5
+    return lib().oracle_tvd2(_p(v))
 
 
 def fast_speeds(gamma, q, d):

@@ -104,6 +104,23 @@ double mp5(const double v[5]) {
     return vor + minmod2(vmin - vor, vmax - vor);
 }
 
+// "Linear reconstruction rather than MP5": v_{i+1/2}^L = v_i + sigma_i / 2 with the limited slope
+// sigma_i = MC(v_i - v_{i-1}, v_{i+1} - v_i), the monotonized-central limiter
+//   MC(a, b) = minmod(2a, 2b, (a + b)/2)
+// (reading O3b: the paper names no limiter; MC is the choice).  Same argument convention as mp5
+// (v[0] and v[4] are not used), so the mirrored stencil gives the right-biased value.
+double minmod3(double a, double b, double c) {
+    if (a > 0.0 && b > 0.0 && c > 0.0) return std::fmin(a, std::fmin(b, c));
+    if (a < 0.0 && b < 0.0 && c < 0.0) return std::fmax(a, std::fmax(b, c));
+    return 0.0;
+}
+double tvd2(const double v[5]) {
+    const double a = v[2] - v[1], b = v[3] - v[2];
+    return v[2] + 0.5 * minmod3(2.0 * a, 2.0 * b, 0.5 * (a + b));
+}
+// REC of the scheme in force: rec = 5 -> MP5, rec = 2 -> limited linear
+double rec_value(int which, const double v[5]) { return which == 2 ? tvd2(v) : mp5(v); }
+
 // ----------------------------------------------------------------------------------
 // Point physics.  A primitive state is q[8] = (rho, vx, vy, vz, p, Bx, By, Bz).
 // Definitions: D = rho W, S = rho h W^2 v + E x B, U = rho h W^2 - p + (E^2+B^2)/2,
@@ -310,6 +327,7 @@ struct Ctx {
     Grid g;
     double gam, cfl;
     int uct = 1, ho = 1;   // scheme switches
+    int rec = 5, rk = 3;   // REC: 5 = MP5, 2 = limited linear; time stepping: SSP-RK3 or RK2
     State s;
     bool has_state = false;
     double t = 0.0, dt_last = 0.0, amax = 0.0;
@@ -392,8 +410,8 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
                 const Field &f = *rec[v];
                 const double sl[5] = {f[nb[0]], f[nb[1]], f[nb[2]], f[nb[3]], f[nb[4]]};
                 const double sr[5] = {f[nb[5]], f[nb[4]], f[nb[3]], f[nb[2]], f[nb[1]]};  // mirrored
-                qL[slot[v]] = mp5(sl);
-                qR[slot[v]] = mp5(sr);
+                qL[slot[v]] = rec_value(cx.rec, sl);
+                qR[slot[v]] = rec_value(cx.rec, sr);
             }
             double F[5], ex[4], FB[3];
             if (cx.uct) {
@@ -403,8 +421,8 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
                 const Field &f = Bc[d];
                 const double sl[5] = {f[nb[0]], f[nb[1]], f[nb[2]], f[nb[3]], f[nb[4]]};
                 const double sr[5] = {f[nb[5]], f[nb[4]], f[nb[3]], f[nb[2]], f[nb[1]]};
-                qL[5 + d] = mp5(sl);
-                qR[5 + d] = mp5(sr);
+                qL[5 + d] = rec_value(cx.rec, sl);
+                qR[5 + d] = rec_value(cx.rec, sr);
                 hll(gam, qL, qR, d, F, ex, FB);
                 for (int a = 0; a < 3; ++a) r.FB[d][a][i0] = FB[a];
             }
@@ -460,14 +478,14 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
             long nbi[6], nbj[6];
             for (int m = 0; m < 6; ++m) { nbi[m] = g.shift(c, i, m - 2); nbj[m] = g.shift(c, j, m - 2); }
             for (int m = 0; m < 5; ++m) { sl[m] = vi_at_j[nbi[m]]; sr[m] = vi_at_j[nbi[5 - m]]; }
-            const double viL = mp5(sl), viR = mp5(sr);
+            const double viL = rec_value(cx.rec, sl), viR = rec_value(cx.rec, sr);
             for (int m = 0; m < 5; ++m) { sl[m] = s.Bf[j][nbi[m]]; sr[m] = s.Bf[j][nbi[5 - m]]; }
-            const double BjL = mp5(sl), BjR = mp5(sr);
+            const double BjL = rec_value(cx.rec, sl), BjR = rec_value(cx.rec, sr);
             // second bracket: i-face quantities reconstructed along j
             for (int m = 0; m < 5; ++m) { sl[m] = vj_at_i[nbj[m]]; sr[m] = vj_at_i[nbj[5 - m]]; }
-            const double vjL = mp5(sl), vjR = mp5(sr);
+            const double vjL = rec_value(cx.rec, sl), vjR = rec_value(cx.rec, sr);
             for (int m = 0; m < 5; ++m) { sl[m] = s.Bf[i][nbj[m]]; sr[m] = s.Bf[i][nbj[5 - m]]; }
-            const double BiL = mp5(sl), BiR = mp5(sr);
+            const double BiL = rec_value(cx.rec, sl), BiR = rec_value(cx.rec, sr);
             // edge speeds: max over the two faces adjacent to the edge
             const long cj = g.shift(c, j, 1), ci = g.shift(c, i, 1);
             const double aip = std::fmax(ap[i][i0], ap[i][cj]), aim = std::fmax(am[i][i0], am[i][cj]);
@@ -524,6 +542,32 @@ void rk3_step(Ctx &cx, double t_end) {
             s.U[v][c] = (1.0 / 3.0) * s0.U[v][c] + (2.0 / 3.0) * (s.U[v][c] + dt * r.U[v][c]);
         for (int v = 0; v < 3; ++v)
             s.Bf[v][c] = (1.0 / 3.0) * s0.Bf[v][c] + (2.0 / 3.0) * (s.Bf[v][c] + dt * r.B[v][c]);
+    }
+    cx.t += dt;
+    cx.dt_last = dt;
+    ++cx.steps;
+}
+
+// "Second order time-stepping": the two-stage SSP Runge-Kutta scheme (Heun),
+//   U1 = U^n + dt L(U^n),  U^{n+1} = 1/2 U^n + 1/2 (U1 + dt L(U1)),   dt as in rk3_step (S9).
+void rk2_step(Ctx &cx, double t_end) {
+    const Grid &g = cx.g;
+    State &s = cx.s;
+    State s0 = s;
+    Rhs r;
+    compute_rhs(cx, s, r);
+    cx.amax = r.amax;
+    double hmin = std::fmin(g.h[0], std::fmin(g.h[1], g.h[2]));
+    double dt = cx.cfl * hmin / r.amax;
+    if (cx.t + dt > t_end) dt = t_end - cx.t;
+    for (long c = 0; c < g.N; ++c) {
+        for (int v = 0; v < 5; ++v) s.U[v][c] = s0.U[v][c] + dt * r.U[v][c];
+        for (int v = 0; v < 3; ++v) s.Bf[v][c] = s0.Bf[v][c] + dt * r.B[v][c];
+    }
+    compute_rhs(cx, s, r);
+    for (long c = 0; c < g.N; ++c) {
+        for (int v = 0; v < 5; ++v) s.U[v][c] = 0.5 * s0.U[v][c] + 0.5 * (s.U[v][c] + dt * r.U[v][c]);
+        for (int v = 0; v < 3; ++v) s.Bf[v][c] = 0.5 * s0.Bf[v][c] + 0.5 * (s.Bf[v][c] + dt * r.B[v][c]);
     }
     cx.t += dt;
     cx.dt_last = dt;
@@ -607,6 +651,18 @@ int oracle_set_scheme(void *h, int uct, int ho) {
     return 0;
 }
 
+// Order switches of P:L304 ("second order time-stepping and linear reconstruction rather than MP5"); call before
+// oracle_set_primitives.  rec: 5 = MP5 (default), 2 = limited linear (MC); rk: 3 = SSP-RK3 (default), 2 = SSP-RK2.
+int oracle_set_order(void *h, int rec, int rk) {
+    Ctx *cx = static_cast<Ctx *>(h);
+    if (!cx || cx->has_state) return -4;
+    if ((rec != 5 && rec != 2) || (rk != 3 && rk != 2)) return -1;
+    cx->rec = rec;
+    cx->rk = rk;
+    return 0;
+}
+double oracle_tvd2(const double v[5]) { return tvd2(v); }
+
 // faces from an edge potential with the second-order (HO=NO) or sixth-order curl
 int oracle_faces_from_potential_ho(int nx, int ny, int nz, int ho, const double *ax, const double *ay, const double *az,
                                    double *bx, double *by, double *bz) {
@@ -651,7 +707,8 @@ int oracle_step(void *h, int nsteps, double t_end) {
     int done = 0;
     for (int s = 0; s < nsteps; ++s) {
         if (!(cx->t < t_end)) break;
-        rk3_step(*cx, t_end);
+        if (cx->rk == 2) rk2_step(*cx, t_end);
+        else rk3_step(*cx, t_end);
         ++done;
     }
     return done;
