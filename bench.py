@@ -51,7 +51,15 @@ ALGO_CC = {
     "k_flux_y": {"flop": 674, "dbl": 24},
     "k_flux_z": {"flop": 674 + 48 * 2 / 3.0, "dbl": (24 + 40 + 40) / 3.0},
 }
-SCHEMES = {"uct-ho": (True, True), "uct-lo": (True, False), "cc-ho": (False, True), "cc-lo": (False, False)}
+# name -> (uct, ho, rec, rk); "*-lo2" is the second-order variant of P:L304 (limited linear REC + SSP-RK2)
+SCHEMES = {"uct-ho": (True, True, 5, 3), "uct-lo": (True, False, 5, 3), "cc-ho": (False, True, 5, 3),
+           "cc-lo": (False, False, 5, 3), "uct-lo2": (True, False, 2, 2), "cc-lo2": (False, False, 2, 2)}
+# the same per-launch words for the two-stage scheme (stage 1 + one fused stage instead of two)
+# the paper's step rates x 512^3 cells for the diagonal CPA wave at 512^3 on ONE NODE of
+# LEONARDO (4 x A100 64 GB), per scheme (Table 1).  vs_baseline is quoted only for that workload.
+PAPER_512_PER_NODE = {"uct-ho": 1.13 * 512 ** 3, "cc-lo": 1.21 * 512 ** 3, "cc-lo2": 2.2e8}
+ALGO_RK2 = {"k_prim": (16 + 26) / 2.0, "k_flux_z": (22 + 32) / 2.0, "k_update": (9 + 12) / 2.0}
+ALGO_CC_RK2 = {"k_prim": (16 + 32) / 2.0, "k_flux_z": (24 + 40) / 2.0}
 
 
 def measured_peaks():
@@ -185,12 +193,16 @@ def run_gpu(args):
 
     n, K, W = args.n, args.steps, max(args.warmup, 3)
     N = n ** 3
-    uct, ho = SCHEMES[args.scheme]
+    uct, ho, rec, rk = SCHEMES[args.scheme]
     if args.scheme != "uct-ho" and (args.workload != "cpa" or args.decompose):
         raise SystemExit("--scheme variants are wired for the default cpa workload only")
-    ALGO = globals()["ALGO"] if uct else ALGO_CC
-    FLOP_PER_CELL_UPDATE = 3 * sum(v["flop"] for v in ALGO.values())
-    BYTES_PER_CELL_UPDATE = 8 * 3 * sum(v["dbl"] for v in ALGO.values())
+    ALGO = {k: dict(v) for k, v in (globals()["ALGO"] if uct else ALGO_CC).items()}
+    if rk == 2:
+        for k, dbl in (ALGO_RK2 if uct else ALGO_CC_RK2).items():
+            ALGO[k]["dbl"] = dbl
+    # (the flop entries are the nominal counts of the MP5 scheme; with linear REC they overstate the arithmetic)
+    FLOP_PER_CELL_UPDATE = rk * sum(v["flop"] for v in ALGO.values())
+    BYTES_PER_CELL_UPDATE = 8 * rk * sum(v["dbl"] for v in ALGO.values())
     decomposed = bool(args.decompose) and world > 1
     if decomposed:
         # ONE periodic box of (n px, n py, n pz) cells, one n^3 block (+ width-8 halos) per rank: halo exchange of
@@ -227,7 +239,7 @@ def run_gpu(args):
         parallelism = "replicas x%d (no collective)" % world
     else:
         w = inputs.cpa_wave(n, n, n, direction=args.direction)
-        e = binding.Echo(n, n, n, GAMMA, CFL, uct=uct, ho=ho)
+        e = binding.Echo(n, n, n, GAMMA, CFL, uct=uct, ho=ho, rec=rec, rk=rk)
         stepper = e.step
         parallelism = "replicas x%d (no collective)" % world
     setk = SETK if uct else "rho vx vy vz p bx by bz".split()       # UCT = NO evolves the cell-centred B
@@ -282,7 +294,7 @@ def run_gpu(args):
         # step (PCIe, both directions) overlap the kernels of the other; every step still moves all its bytes
         side = torch.cuda.Stream()
         with torch.cuda.stream(side):
-            e_b = binding.Echo(*e.n, GAMMA, CFL, uct=uct, ho=ho)
+            e_b = binding.Echo(*e.n, GAMMA, CFL, uct=uct, ho=ho, rec=rec, rk=rk)
         outs_b = [torch.empty(e.shape, dtype=torch.float64).pin_memory() for _ in range(8)]
         lanes = [(e, outs), (e_b, outs_b)]
         for h, o in lanes:
@@ -349,18 +361,25 @@ def run_gpu(args):
         cpu = {"value": rate, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
                "sample": "%d^3 box of the same CPA wave, %d RK3 steps, %.1f s, single thread" % (args.cpu_n, args.cpu_steps, dt)}
 
+    vs_baseline, baseline_note = None, None
+    if args.workload == "cpa" and n == 512 and args.direction == "diag" and not decomposed and args.scheme in PAPER_512_PER_NODE:
+        vs_baseline = value / PAPER_512_PER_NODE[args.scheme]
+        baseline_note = ("paper: %.3g cell-updates/s on one LEONARDO node (4 x A100 64 GB) for this workload and scheme "
+                         "(BASELINE.md section 1); this run: %d x B200" % (PAPER_512_PER_NODE[args.scheme], world))
     nlaunch = sum(cnt for _, cnt in ktimes.values())
     line = {"metric": "fp64_cell_updates_per_sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": vs_baseline, "dtype": "f64", "data": "synthetic",
             "config": {"workload": {"turb2d": "turbulence_2.5d_%d^2" % n, "turb3d": "alfvenic_turbulence_%d^3" % n}.get(
                            args.workload, "cpa_wave_%s_%d^3" % (args.direction, n)),
                        "grid": list(e.n), "gamma": GAMMA, "cfl": CFL,
                        "scheme": {"uct-ho": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)",
                                   "uct-lo": "MP5+HLL+UCT+SSPRK3, second-order INT/DER (UCT=YES, HO=NO)",
                                   "cc-ho": "MP5+HLL+DER6+SSPRK3, cell-centred B (UCT=NO, HO=YES)",
-                                  "cc-lo": "MP5+HLL+SSPRK3, cell-centred B (UCT=HO=NO)"}[args.scheme], "cells": N,
-                       "parallelism": parallelism,
+                                  "cc-lo": "MP5+HLL+SSPRK3, cell-centred B (UCT=HO=NO)",
+                                  "uct-lo2": "linear(MC)+HLL+UCT+SSPRK2, second-order INT/DER (UCT=YES, HO=NO)",
+                                  "cc-lo2": "linear(MC)+HLL+SSPRK2, cell-centred B (UCT=HO=NO)"}[args.scheme], "cells": N,
+                       "parallelism": parallelism, "baseline_note": baseline_note,
                        "cache": "working set %.1f GB per GPU, far larger than the 126 MB L2" % (44 * 8 * N / 1e9)},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "cell-updates/s", "steps": Ke, "serial_value": e2e_serial,
@@ -407,7 +426,8 @@ def main():
                     help="cpa: BASELINE.json configs (default); turb2d: the paper's 2.5-D turbulence on n x n x 1")
     ap.add_argument("--scheme", default="uct-ho", choices=sorted(SCHEMES),
                     help="the paper's switches (P:L124, L138): uct-ho = UCT=HO=YES (default, the headline), "
-                         "uct-lo = HO=NO, cc-ho / cc-lo = UCT=NO with the cell-centred B (row f2)")
+                         "uct-lo = HO=NO, cc-ho / cc-lo = UCT=NO with the cell-centred B, *-lo2 = limited linear "
+                         "REC + SSP-RK2 (P:L304) (row f2)")
     ap.add_argument("--decompose", action="store_true",
                     help="N > 1: one decomposed box (n^3 cells per rank, halo exchange) instead of N replicas")
     args = ap.parse_args()

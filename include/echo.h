@@ -55,6 +55,15 @@ echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl);
  * Defaults: uct = 1, ho = 1. */
 int echo_set_scheme(echo_ctx *ctx, int uct, int ho);
 
+/* Host only.  The second-order variant the paper quotes a throughput for ("second order time-stepping and
+ * linear reconstruction rather than MP5"), to be called before echo_set_primitives and after echo_set_scheme.
+ * rec = 5: MP5 (default); rec = 2: v_i + MC(v_i - v_{i-1}, v_{i+1} - v_i)/2 with the monotonized-central slope
+ * MC(a, b) = minmod(2a, 2b, (a+b)/2) (reading O3b), used by the sweeps and by UCT; built with the
+ * second-order INT/DER only: ECHO_EINVAL unless echo_set_scheme(ctx, uct, 0) was called first.
+ * rk = 3: SSP-RK3 (default); rk = 2: U1 = U^n + dt L(U^n), U^{n+1} = (U^n + U1 + dt L(U1))/2, dt as for RK3.
+ * Block handles (echo_create_block) accept (5, 3) only.  ECHO_EINVAL on other values, ECHO_ESTATE once a state exists. */
+int echo_set_order(echo_ctx *ctx, int rec, int rk);
+
 /* Host only.  Frees the handle (never the workspace). */
 void echo_destroy(echo_ctx *ctx);
 

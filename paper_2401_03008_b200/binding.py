@@ -21,6 +21,7 @@ SIGNATURES = {
     "echo_create": (_vp, [_int, _int, _int, _dbl, _dbl]),
     "echo_destroy": (None, [_vp]),
     "echo_set_scheme": (_int, [_vp, _int, _int]),
+    "echo_set_order": (_int, [_vp, _int, _int]),
     "echo_workspace_bytes": (_sz, [_vp]),
     "echo_bind": (_int, [_vp, _vp, _sz, _vp]),
     "echo_last_error": (C.c_char_p, [_vp]),
@@ -101,7 +102,7 @@ class EchoError(RuntimeError):
 class Echo:
     """One periodic unit box on the current CUDA device.  Tensors are torch.float64, shape (nz, ny, nx)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True, uct=True):
+    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True, uct=True, rec=5, rk=3):
         """block = (gnx, gny, gnz, halo_x, halo_y, halo_z): a domain-decomposition block (echo_create_block).
         ho / uct: the paper's scheme switches (echo_set_scheme); with uct=False the three "face" arrays of
         set_primitives / get_primitives are the cell-centred B."""
@@ -119,6 +120,8 @@ class Echo:
             raise ValueError("echo_create: bad arguments")
         if not (ho and uct):
             self._check(self.L.echo_set_scheme(self.h, int(bool(uct)), int(bool(ho))))
+        if (rec, rk) != (5, 3):     # echo_set_order: 2 / 2 = limited linear REC + SSP-RK2
+            self._check(self.L.echo_set_order(self.h, int(rec), int(rk)))
         nbytes = self.L.echo_workspace_bytes(self.h)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned by the caller side
         self._check(self.L.echo_bind(self.h, self.workspace.data_ptr(), nbytes, _stream()))

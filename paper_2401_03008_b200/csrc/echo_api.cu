@@ -24,6 +24,7 @@ struct echo_ctx {
     double *field[NFIELD] = {nullptr};
     long long npad = 0;
     bool bound = false, has_state = false;
+    int rk = 3;              // SSP-RK3 or SSP-RK2 (echo_set_order)
     bool block = false;      // echo_create_block: explicit spacing, halos refreshed by the caller between stages
     std::string err;
     // measurement aids (echo_timing / echo_get_timing)
@@ -115,7 +116,13 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
     if (g.n[D] == 1) {   // a one-cell axis: no stencil work left, only the face quantities (k_flux_flat)
-        if (g.uct)
+        if (g.rec == 2 && g.uct)
+            KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE, true, 2><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
+                   g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        else if (g.rec == 2)
+            KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE, false, 2><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
+                   g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        else if (g.uct)
             KL(KC_FLUX + D, "k_flux_flat", k_flux_flat<D, MODE><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(
                    g, st, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
         else
@@ -130,7 +137,11 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
     if (!g.uct) {   // UCT = NO: 8 flux components, rings of 49 KB in dynamic shared memory
         constexpr int R = NT / T, RL = 3 * R, SB = RL + 4;   // as in k_flux
         constexpr size_t smem = sizeof(double) * ((D == 0) ? (8 + 8) * T * SB : RL * (8 + 8) * T);
-        if (g.ho) {
+        if (g.rec == 2) {   // linear REC is wired with the second-order INT/DER only (echo_set_order)
+            auto kern = k_flux<D, NT, MODE, false, false, 2>;
+            CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            KL(KC_FLUX + D, "k_flux_cc", kern<<<grid, NT, smem, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+        } else if (g.ho) {
             auto kern = k_flux<D, NT, MODE, true, false>;
             CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             KL(KC_FLUX + D, "k_flux_cc", kern<<<grid, NT, smem, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
@@ -141,7 +152,9 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
         }
         return ECHO_OK;
     }
-    if (g.ho)
+    if (g.rec == 2)
+        KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, false, true, 2><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
+    else if (g.ho)
         KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, true><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
     else
         KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, false><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
@@ -201,7 +214,8 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
         nchunk = std::max(1, std::min(nchunk, (g.n[2] + 15) / 16));
         const int CZ = (g.n[2] + nchunk - 1) / nchunk;
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
-        KL(KC_UCT, "k_uct2", k_uct2<<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
+        if (g.rec == 2) KL(KC_UCT, "k_uct2", k_uct2<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
+        else KL(KC_UCT, "k_uct2", k_uct2<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
     }
     return ECHO_OK;
 }
@@ -266,6 +280,7 @@ echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl) {
     for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; g.lo[d] = 0; g.hi[d] = g.n[d]; }
     g.ho = 1;
     g.uct = 1;
+    g.rec = 5;
     c->gamma = gamma;
     c->cfl = cfl;
     c->gg = gamma / (gamma - 1.0);
@@ -356,6 +371,7 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     if (rc) return rc;
     if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    const bool rk2 = ctx->rk == 2;   // SSP-RK2 (O3b): stage 1 as below, then U^{n+1} = 1/2 U^n + 1/2 (U1 + dt L(U1))
     if (!ctx->g.uct) {
         // UCT = NO: all 8 fields are cell fields.  Stage 1 writes rhs only; its update is formed by the
         // k_prim of stage 2 (U and B); stages 2 and 3 combine all 8 fields inside their z-sweep.  10 launches.
@@ -364,10 +380,12 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
             if ((rc = launch_operator(ctx, s0, 2))) return rc;
             Stage s12 = s1;
             for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];
-            const StagePlan p2 = {true, true, 1, 1, 0.75, 0.25};
+            const StagePlan p2 = {true, true, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25};
             if ((rc = launch_operator(ctx, s12, 0, &p2))) return rc;
-            const StagePlan p3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
-            if ((rc = launch_operator(ctx, s1, 0, &p3))) return rc;
+            if (!rk2) {
+                const StagePlan p3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
+                if ((rc = launch_operator(ctx, s1, 0, &p3))) return rc;
+            }
             KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
         }
         return ECHO_OK;
@@ -382,12 +400,12 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
         {
             Stage s12 = s1;                       // operator state: faces from the stage buffers ...
             for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];   // ... cell fields = U^n (+ dt R inside k_prim)
-            const StagePlan pl = {true, true, 1, 1, 0.75, 0.25};
+            const StagePlan pl = {true, true, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25};
             if ((rc = launch_operator(ctx, s12, 0, &pl))) return rc;
-            if ((rc = launch_update(ctx, s1, 1, 1, 0.75, 0.25, false))) return rc;
+            if ((rc = launch_update(ctx, s1, 1, rk2 ? 0 : 1, pl.c0, pl.c1, false))) return rc;
         }
         // stage 3: U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
-        {
+        if (!rk2) {
             const StagePlan pl = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
             if ((rc = launch_operator(ctx, s1, 0, &pl))) return rc;
             if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false))) return rc;
@@ -596,9 +614,22 @@ echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, in
     return c;
 }
 
+int echo_set_order(echo_ctx *ctx, int rec, int rk) {
+    if (!ctx) return ECHO_EINVAL;
+    if (ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_order must precede echo_set_primitives");
+    if ((rec != 5 && rec != 2) || (rk != 3 && rk != 2)) return fail(ctx, ECHO_EINVAL, "rec must be 5 or 2, rk 3 or 2");
+    if (ctx->block && (rec != 5 || rk != 3)) return fail(ctx, ECHO_EINVAL, "block handles run MP5 + SSP-RK3 only");
+    if (rec == 2 && ctx->g.ho)
+        return fail(ctx, ECHO_EINVAL, "linear reconstruction is built with the second-order INT/DER: echo_set_scheme(ctx, uct, 0) first");
+    ctx->g.rec = rec;
+    ctx->rk = rk;
+    return ECHO_OK;
+}
+
 int echo_set_scheme(echo_ctx *ctx, int uct, int ho) {
     if (!ctx) return ECHO_EINVAL;
     if (ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_scheme must precede echo_set_primitives");
+    if (ho && ctx->g.rec == 2) return fail(ctx, ECHO_EINVAL, "HO=YES with linear reconstruction is not built (echo_set_order)");
     if (!uct && ctx->block) return fail(ctx, ECHO_EINVAL, "UCT=NO is not built for block handles (echo_create_block)");
     ctx->g.uct = uct ? 1 : 0;
     ctx->g.ho = ho ? 1 : 0;
@@ -624,7 +655,7 @@ int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
-    if (!ctx->g.uct) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES only");
+    if (!ctx->g.uct || ctx->rk != 3) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES and SSP-RK3 only");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     if (stage == 1) {
         KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
@@ -639,7 +670,7 @@ int echo_stage_finish(echo_ctx *ctx, int stage) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
-    if (!ctx->g.uct) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES only");
+    if (!ctx->g.uct || ctx->rk != 3) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES and SSP-RK3 only");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     if (stage == 1) {
         // dt from the (all-reduced) a_max, UCT, then the UNFUSED update of all 8 fields: U1 must exist in

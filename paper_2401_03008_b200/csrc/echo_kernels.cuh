@@ -192,7 +192,7 @@ struct FluxUpd { const double *base[8]; const double *cur[8]; double *out[8]; do
 // like the other conserved variables: 8 reconstructed fields, 8 flux components (rhs of B in st.E), no face
 // quantities for UCT.  The inputs are the k_prim copies st.Bc, not the evolved st.Bf: the fused RK update of
 // MODE 1 overwrites the evolved B while wrapped rows of it are still to be read.  Compile-time branches only: the UCT = true instantiations are the kernel described above.
-template <int D, int NT, int MODE, bool HO, bool UCT = true>
+template <int D, int NT, int MODE, bool HO, bool UCT = true, int REC = 5>
 __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
                                              int want_amax, FluxUpd up) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
             for (int v = 0; v < (UCT ? 7 : 8); ++v) {
                 const double *p = Pb + v * SV;
                 const double s0 = p[sl[0]], s1 = p[sl[1]], s2 = p[sl[2]], s3 = p[sl[3]], s4 = p[sl[4]], s5 = p[sl[5]];
-                mp5_pair<true>(s0, s1, s2, s3, s4, s5, qL[slot[v]], qR[slot[v]]);
+                rec_pair<REC>(s0, s1, s2, s3, s4, s5, qL[slot[v]], qR[slot[v]]);
             }
             double F[NC], ap, am, vb1 = 0.0, vb2 = 0.0;
             if (UCT) {
@@ -357,7 +357,7 @@ __global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double 
 // face quantities UCT needs (a+, a-, vbar), a_max and, in MODE 1, the RK combination remain.  The arithmetic of
 // the face is the generic one applied to six equal stencil values, so a flat run stays bit-identical to the same
 // data on a thicker grid (dimensional-reduction test).
-template <int D, int MODE, bool UCT = true>
+template <int D, int MODE, bool UCT = true, int REC = 5>
 __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam, double gg, Ctrl *ctrl, int want_amax,
                                                    FluxUpd up) {
     constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
@@ -375,7 +375,7 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
 #pragma unroll
         for (int v = 0; v < (UCT ? 7 : 8); ++v) {
             const double s = __ldg(rec[v] + c);
-            mp5_pair<true>(s, s, s, s, s, s, qL[slot[v]], qR[slot[v]]);
+            rec_pair<REC>(s, s, s, s, s, s, qL[slot[v]], qR[slot[v]]);
         }
         double F[NC], ap, am, vb1, vb2;
         if (UCT) {

@@ -178,6 +178,28 @@ __device__ __forceinline__ void mp5_pair(double s0, double s1, double s2, double
 #endif
 }
 
+// O3b — the second-order REC of P:L304: v_i + MC(a, b)/2 with the monotonized-central slope
+// MC(a, b) = minmod(2a, 2b, (a + b)/2); both one-sided values at the face between s2 and s3.
+__device__ __forceinline__ double mc_slope(double a, double b) {
+    const double s = 0.5 * (a + b);
+    double m = (fabs(a) < fabs(b)) ? a : b;      // same sign: 2 min(|a|, |b|) against |a + b|/2
+    m = 2.0 * m;
+    m = (fabs(s) < fabs(m)) ? s : m;
+    return ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
+}
+__device__ __forceinline__ void tvd2_pair(double s1, double s2, double s3, double s4, double &L, double &R) {
+    const double b = s3 - s2;
+    L = s2 + 0.5 * mc_slope(s2 - s1, b);
+    R = s3 - 0.5 * mc_slope(b, s4 - s3);
+}
+// REC of the scheme in force
+template <int REC>
+__device__ __forceinline__ void rec_pair(double s0, double s1, double s2, double s3, double s4, double s5, double &L,
+                                         double &R) {
+    if (REC == 2) tvd2_pair(s1, s2, s3, s4, L, R);
+    else mp5_pair<true>(s0, s1, s2, s3, s4, s5, L, R);
+}
+
 // Branch-free first half of mp5_pair: the two unlimited values and the two S&H test bits (bit 0: L needs the
 // limiter, bit 1: R); mp5_pair_fix applies the limiter afterwards.  Used where several stencils should be
 // interleaved by the compiler before any branch (k_uct2).

@@ -17,6 +17,7 @@ struct Grid {
     // scheme switches of the paper (echo_set_scheme): ho = 0 makes INT and DER second order;
     // uct = 0 evolves a cell-centred B like the other conserved variables
     int ho, uct;
+    int rec;                  // REC: 5 = MP5, 2 = limited linear (MC), echo_set_order
 };
 
 // Device control block (first bytes of the workspace).  Everything echo_step needs between

@@ -30,6 +30,8 @@ __device__ __forceinline__ double uct_hll(double ap, double am, double vL, doubl
     return (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) * rcp_fast(ap + am);
 }
 
+// LIN: the limited linear REC of O3b instead of MP5 (echo_set_order)
+template <bool LIN = false>
 __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
     __shared__ double sXR[2][4][UCT_XR];
     __shared__ double sYR[2][4][UCT_YR];
@@ -138,6 +140,11 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
             // one upwinded product at a time: MP5 L/R (O3) of (vbar, B) to the edge, then O7
             auto bracket = [&](const double *p, const double *q, int S, double ap, double am) {
                 double vL, vR, BL, BR;
+                if (LIN) {
+                    tvd2_pair(p[S], p[2 * S], p[3 * S], p[4 * S], vL, vR);
+                    tvd2_pair(q[S], q[2 * S], q[3 * S], q[4 * S], BL, BR);
+                    return uct_hll(ap, am, vL, vR, BL, BR);
+                }
                 const unsigned nv = mp5_pair_fast(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
                 const unsigned nb = mp5_pair_fast(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
                 if (nv | nb) {

@@ -386,3 +386,41 @@ def test_uct_no_variant(torch, eb, ob, shape, ho):
     assert blk.L.echo_set_scheme(blk.h, 0, 1) == eb.ECHO_EINVAL   # block handles: UCT=YES only
     with pytest.raises(eb.EchoError):
         e.stage_sweeps(1)
+
+
+@pytest.mark.parametrize("shape,uct,rec,rk", [((40, 24, 20), True, 2, 2), ((40, 24, 20), False, 2, 2), ((33, 1, 7), True, 2, 2),
+                                               ((19, 21, 1), False, 2, 2), ((24, 20, 16), True, 5, 2), ((24, 20, 16), False, 2, 3)])
+def test_second_order_variant(torch, eb, ob, shape, uct, rec, rk):
+    """Row f2, the second-order variant of P:L304 (limited linear REC with the MC slope, SSP-RK2; reading O3b): L(U)
+    and 6 steps against the oracle run with the same switches, for the staggered and the cell-centred B."""
+    ho = rec == 5
+    w = inputs.turbulence(None, shape=shape)
+    nx, ny, nz = shape
+    bsm = ob.faces_from_potential(w["ax"], w["ay"], w["az"], ho=ho)
+    b = [bsm[d] + w["b0"][d] for d in range(3)]
+    if not uct:
+        z, y, x = np.meshgrid((np.arange(nz) + 0.5) / nz, (np.arange(ny) + 0.5) / ny, (np.arange(nx) + 0.5) / nx, indexing="ij")
+        b = [b[d] + 0.05 * np.cos(2 * np.pi * (x + 2 * y + 3 * z) + d) for d in range(3)]
+    args = [w[k] for k in ("rho", "vx", "vy", "vz", "p")] + b
+    o = ob.Oracle(*shape, G, 0.3, uct=uct, ho=ho, rec=rec, rk=rk)
+    o.set_primitives(*args)
+    e = eb.Echo(*shape, G, 0.3, uct=uct, ho=ho, rec=rec, rk=rk)
+    e.set_primitives(*[dev(torch, a) for a in args])
+    rg, ro = e.rhs(), o.rhs()
+    for name in ("rhsU", "rhsB", "E"):
+        for c in range(len(ro[name])):
+            assert absinf(rg[name][c].cpu().numpy(), ro[name][c]) <= 1e-11 * max(1.0, np.abs(ro[name][c]).max()), (name, c)
+    e.step(6)
+    o.step(6)
+    compare_prims(e, o, tight=1e-11)
+    dg, do = e.diagnostics(), o.diagnostics()
+    assert dg["steps"] == 6 and dg["t"] == pytest.approx(do["t"], rel=1e-13) and dg["c2p_failures"] == 0
+    if uct:
+        assert e.div_b() <= 1e-11
+    # argument checks of echo_set_order
+    h = eb.Echo(8, 8, 8, G, 0.3)
+    assert h.L.echo_set_order(h.h, 2, 3) == eb.ECHO_EINVAL          # linear REC needs HO=NO first
+    assert h.L.echo_set_order(h.h, 4, 3) == eb.ECHO_EINVAL and h.L.echo_set_order(h.h, 5, 1) == eb.ECHO_EINVAL
+    assert h.L.echo_set_order(h.h, 5, 2) == eb.ECHO_OK
+    with pytest.raises(eb.EchoError):
+        e._check(e.L.echo_set_order(e.h, 5, 3))                     # too late: the state exists
