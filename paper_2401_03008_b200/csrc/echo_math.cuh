@@ -103,6 +103,16 @@ __device__ __forceinline__ double mp5_limit(double vm2, double vm1, double v0, d
 __device__ __noinline__ double mp5_limit_call(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
     return mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
 }
+// the same behind the exact S&H test (for callers that flagged the stencil with a cheaper superset of it)
+__device__ __noinline__ double mp5_limit_call_checked(double vm2, double vm1, double v0, double vp1, double vp2,
+                                                      double vor) {
+    const double t = vor - v0;
+    const double a = vp1 - v0, b = 4.0 * (v0 - vm1);
+    const double m = (fabs(a) < fabs(b)) ? a : b;
+    const double mm = ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
+    if (!(t * (t - mm) > 1e-10)) return vor;
+    return mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
+}
 // INL: limiter inlined behind a branch (flux sweeps) or called out of line (UCT kernel, whose 24
 // reconstructions would otherwise overflow the instruction cache).
 template <bool INL = true>
@@ -132,7 +142,7 @@ __device__ __forceinline__ double times4(double d) {
 }
 #ifndef ECHO_SH_SUPERSET
 #define ECHO_SH_SUPERSET 1       // sweeps: x 0.785 -> 0.776, y 0.757 -> 0.741, z 0.808 -> 0.804 ms at 256^3
-#define ECHO_SH_SUPERSET_UCT 0
+#define ECHO_SH_SUPERSET_UCT 0   // k_uct2: 1.16 -> 1.19-1.22 ms with it (inline or behind the checked call)
 #endif
 template <bool INL = true>
 __device__ __forceinline__ void mp5_pair(double s0, double s1, double s2, double s3, double s4, double s5, double &L,
@@ -209,7 +219,7 @@ __device__ __forceinline__ unsigned mp5_pair_fast(double s0, double s1, double s
     R = (3.0 / 128.0) * s5 + ((-20.0 / 128.0) * s4 + ((90.0 / 128.0) * s3 + ((60.0 / 128.0) * s2 + (-5.0 / 128.0) * s1)));
     const double d23 = s3 - s2;
     const double tL = L - s2, tR = R - s3;
-#if ECHO_SH_SUPERSET_UCT   // measured in k_uct2: 1.22 ms against 1.16 ms (162 registers), so off there
+#if ECHO_SH_SUPERSET_UCT
     // superset of the S&H test (see mp5_pair); mp5_pair_fix repeats the exact test
     return ((tL * (tL - d23) > 1e-10 || tL * fma(-4.0, s2 - s1, tL) > 1e-10) ? 1u : 0u) |
            ((tR * (tR + d23) > 1e-10 || tR * fma(-4.0, s3 - s4, tR) > 1e-10) ? 2u : 0u);
@@ -221,15 +231,9 @@ __device__ __forceinline__ unsigned mp5_pair_fast(double s0, double s1, double s
 }
 __device__ __forceinline__ void mp5_pair_fix(unsigned bits, double s0, double s1, double s2, double s3, double s4,
                                              double s5, double &L, double &R) {
-#if ECHO_SH_SUPERSET_UCT   // measured in k_uct2: 1.22 ms against 1.16 ms (162 registers), so off there
-    if (bits & 1u) {
-        const double tL = L - s2;
-        if (tL * (tL - minmod2(s3 - s2, times4(s2 - s1))) > 1e-10) L = mp5_limit_call(s0, s1, s2, s3, s4, L);
-    }
-    if (bits & 2u) {
-        const double tR = R - s3;
-        if (tR * (tR - minmod2(s2 - s3, times4(s3 - s4))) > 1e-10) R = mp5_limit_call(s5, s4, s3, s2, s1, R);
-    }
+#if ECHO_SH_SUPERSET_UCT
+    if (bits & 1u) L = mp5_limit_call_checked(s0, s1, s2, s3, s4, L);
+    if (bits & 2u) R = mp5_limit_call_checked(s5, s4, s3, s2, s1, R);
 #else
     if (bits & 1u) L = mp5_limit_call(s0, s1, s2, s3, s4, L);
     if (bits & 2u) R = mp5_limit_call(s5, s4, s3, s2, s1, R);
