@@ -290,33 +290,38 @@ def run_gpu(args):
     e2e_serial, _ = whole_job_rate(N, Ke, ev0.elapsed_time(ev1), "cuda", world)
     e2e_value, e2e_how = e2e_serial, "serial: upload, step, download one after the other on one stream"
     if not decomposed:
-        # the same three calls per step, but on TWO handles bound to two streams: the uploads and downloads of one
-        # step (PCIe, both directions) overlap the kernels of the other; every step still moves all its bytes
-        side = torch.cuda.Stream()
-        with torch.cuda.stream(side):
-            e_b = binding.Echo(*e.n, GAMMA, CFL, uct=uct, ho=ho, rec=rec, rk=rk)
-        outs_b = [torch.empty(e.shape, dtype=torch.float64).pin_memory() for _ in range(8)]
-        lanes = [(e, outs), (e_b, outs_b)]
+        # the same three calls per step, but on L handles bound to L streams: upload (PCIe H2D), kernels and download
+        # (PCIe D2H) of consecutive steps overlap; every step still moves all its bytes.  Three stages need three
+        # lanes to keep the slowest one (a PCIe direction) busy; fewer if the workspaces would not fit.
+        L = max(1, min(args.e2e_lanes, int(150e9 // e.workspace.numel())))
+        sides = [torch.cuda.Stream() for _ in range(L - 1)]
+        lanes = [(e, outs)]
+        for sd in sides:
+            with torch.cuda.stream(sd):
+                h = binding.Echo(*e.n, GAMMA, CFL, uct=uct, ho=ho, rec=rec, rk=rk)
+            lanes.append((h, [torch.empty(e.shape, dtype=torch.float64).pin_memory() for _ in range(8)]))
         for h, o in lanes:
             h.set_primitives_host(*host); h.step(1); h.get_primitives_host(o)
         barrier()
         ev0.record()
         for i in range(Ke):
-            h, o = lanes[i % 2]
-            if i >= 2:
-                h.synchronize()                      # step i-2 of this lane is back before its buffers are reused
+            h, o = lanes[i % L]
+            if i >= L:
+                h.synchronize()                      # step i-L of this lane is back before its buffers are reused
             h.set_primitives_host(*host)
             h.step(1)
             h.get_primitives_host(o, sync=False)
         for h, _ in lanes:
             h.synchronize()
-        torch.cuda.current_stream().wait_stream(side)
+        for sd in sides:
+            torch.cuda.current_stream().wait_stream(sd)
         ev1.record()
         barrier()
         e2e_value, _ = whole_job_rate(N, Ke, ev0.elapsed_time(ev1), "cuda", world)
-        e2e_how = "two handles on two streams: transfers of one step overlap the kernels of the other"
-        assert torch.equal(outs[0], outs_b[0])
-        del e_b
+        e2e_how = "%d handles on %d streams: uploads, kernels and downloads of consecutive steps overlap" % (L, L)
+        for _, o in lanes[1:]:
+            assert torch.equal(outs[0], o[0])
+        del lanes[1:]
     # sanity of what came back: one step of the wave stays within truncation error of the input
     assert abs(float(outs[0].mean()) - 1.0) < (1e-6 if args.workload == "cpa" else 1e-2)
 
@@ -417,7 +422,8 @@ def main():
     ap.add_argument("--impl", default="echo", choices=["echo", "reference"])
     ap.add_argument("--n", type=int, default=256, help="box size n^3 (BASELINE.json configs[2]: 256)")
     ap.add_argument("--direction", default="diag", choices=["diag", "x"])
-    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--e2e-lanes", type=int, default=3, help="handles/streams of the pipelined end-to-end measurement")
     ap.add_argument("--cpu-n", type=int, default=64)
     ap.add_argument("--cpu-steps", type=int, default=6)
     ap.add_argument("--ref-n", type=int, default=48)
