@@ -106,6 +106,15 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
  * speeds of the same step (S9).  No host synchronisation. */
 int echo_step(echo_ctx *ctx, int nsteps, double t_end);
 
+/* Host loop around echo_step: advances until t >= t_end (last dt clipped), max_steps steps were taken, or a
+ * con2prim failure was counted.  echo_step cannot know on the host when t_end is reached, and steps enqueued past
+ * it still run their kernels; this call enqueues chunks sized from the current a_max (at most 2048 steps, about 2 %
+ * more than needed) and reads the 4 KB control block back after each chunk, so it SYNCHRONISES the stream a few
+ * times.  steps_taken_host (host pointer, may be NULL) receives the number of steps actually taken.  Returns
+ * ECHO_EC2P if the run stopped on a con2prim failure, ECHO_EINVAL for NaN / negative arguments and for block
+ * handles. */
+int echo_run_until(echo_ctx *ctx, double t_end, long max_steps, long *steps_taken_host);
+
 /* Runs INT + con2prim on the current state and writes the 8 cell-centred fields; the three face
  * pointers may be NULL.  Does not synchronise.  (con2prim failures are reported by
  * echo_diagnostics, not here, because that would need a synchronisation.) */

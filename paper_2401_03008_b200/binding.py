@@ -29,6 +29,7 @@ SIGNATURES = {
     "echo_set_primitives_host": (_int, [_vp] + [_vp] * 8),
     "echo_faces_from_potential": (_int, [_vp] + [_vp] * 3 + [_dbl] * 3 + [_vp] * 3),
     "echo_step": (_int, [_vp, _int, _dbl]),
+    "echo_run_until": (_int, [_vp, _dbl, C.c_long, C.POINTER(C.c_long)]),
     "echo_get_primitives": (_int, [_vp] + [_vp] * 11),
     "echo_get_primitives_host": (_int, [_vp] + [_vp] * 11),
     "echo_get_primitives_host_async": (_int, [_vp] + [_vp] * 11),
@@ -215,6 +216,12 @@ class Echo:
         """8-byte control word as an int64 tensor view: 0 = a_max bits, 1 = t, 2 = dt, 3 = con2prim failures."""
         off = self.L.echo_ctrl_offset(int(what))
         return self.workspace[off:off + 8].view(_torch().int64)
+
+    def run_until(self, t_end, max_steps=2 ** 31 - 1):
+        """echo_run_until: steps taken (synchronises); raises on a con2prim failure."""
+        n = C.c_long(0)
+        self._check(self.L.echo_run_until(self.h, float(t_end), int(max_steps), C.byref(n)))
+        return n.value
 
     def stage_sweeps(self, stage, t_end=math.inf):
         self._check(self.L.echo_stage_sweeps(self.h, int(stage), float(t_end)))

@@ -415,6 +415,35 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     return ECHO_OK;
 }
 
+int echo_run_until(echo_ctx *ctx, double t_end, long max_steps, long *steps_taken_host) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    if (std::isnan(t_end) || max_steps < 0) return fail(ctx, ECHO_EINVAL, "t_end is NaN or max_steps < 0");
+    if (ctx->block) return fail(ctx, ECHO_EINVAL, "block handles are stepped stage by stage by their owner");
+    Ctrl h;
+    CU(cudaMemcpyAsync(&h, ctx->ctrl, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    const long long steps0 = h.steps;
+    const unsigned long long fails0 = h.c2p_fail_total;
+    while (h.t < t_end && h.steps - steps0 < max_steps && h.c2p_fail_total == fails0) {
+        // echo_step enqueues exactly the steps it is given (those past t_end are device-side no-ops that still
+        // cost their kernels), so the count comes from the current speed: a little more than needed, then look
+        long k = 8;
+        if (h.amax > 0.0 && std::isfinite(t_end)) {
+            const double est = (t_end - h.t) / (ctx->cfl * ctx->hmin / h.amax) * 1.02 + 1.0;
+            k = est < 2048.0 ? (long)std::ceil(est) : 2048;
+        } else if (h.amax > 0.0) {
+            k = 2048;
+        }
+        k = std::max(1L, std::min(k, max_steps - (long)(h.steps - steps0)));
+        if ((rc = echo_step(ctx, (int)k, t_end))) return rc;
+        CU(cudaMemcpyAsync(&h, ctx->ctrl, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    if (steps_taken_host) *steps_taken_host = (long)(h.steps - steps0);
+    return h.c2p_fail_total == fails0 ? ECHO_OK : ECHO_EC2P;
+}
+
 int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, double *vz, double *p, double *bxc,
                         double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
     int rc = check_ready(ctx, true);

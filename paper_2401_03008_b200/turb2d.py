@@ -55,15 +55,11 @@ def main(argv=None):
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for s in range(1, args.samples + 1):
-        # echo_step enqueues exactly the steps it is given (those past t_end are no-ops on the device), so the
-        # count is bounded from the last dt: a few more than needed, then look at the clock
-        target = t_end * s / args.samples
-        while True:
-            d = e.diagnostics()
-            if d["t"] >= target or d["c2p_failures"]:
-                break
-            dt = 0.3 / n / (d["amax"] if d["amax"] > 0.0 else 1.0)     # not dt_last: the last step may have been clipped
-            e.step(min(5000, max(1, int(math.ceil((target - d["t"]) / dt * 1.02)) + 1)), t_end=target)
+        try:
+            e.run_until(t_end * s / args.samples)      # echo_run_until: chunks sized from a_max, stops on t_end
+        except binding.EchoError as err:
+            if err.code != binding.ECHO_EC2P:
+                raise
         q, rec = sample()
         hist.append(rec)
         if rec["c2p_failures"] or not math.isfinite(rec["max_W"]):

@@ -424,3 +424,24 @@ def test_second_order_variant(torch, eb, ob, shape, uct, rec, rk):
     assert h.L.echo_set_order(h.h, 5, 2) == eb.ECHO_OK
     with pytest.raises(eb.EchoError):
         e._check(e.L.echo_set_order(e.h, 5, 3))                     # too late: the state exists
+
+
+def test_run_until_matches_the_oracle_step_count_and_state(torch, eb, ob):
+    """echo_run_until: one period of the diagonal wave at 16^3 takes the oracle's 66 steps (last one clipped), the
+    state is the one echo_step gives, max_steps is honoured and a second call at the same t_end does nothing."""
+    n = 16
+    w = inputs.cpa_wave(n, n, n)
+    o = ob.Oracle(n, n, n, G, 0.3)
+    o.set_primitives(*[w[k] for k in SETK])
+    assert o.step(10 ** 6, w["T"]) == 66
+    e = eb.Echo(n, n, n, G, 0.3)
+    e.set_primitives(*[dev(torch, w[k]) for k in SETK])
+    assert e.run_until(w["T"], max_steps=10) == 10
+    assert e.diagnostics()["steps"] == 10
+    assert e.run_until(w["T"]) == 56
+    d = e.diagnostics()
+    assert d["steps"] == 66 and d["t"] == w["T"]
+    compare_prims(e, o, tight=1e-11)
+    assert e.run_until(w["T"]) == 0 and e.diagnostics()["steps"] == 66
+    assert e.L.echo_run_until(e.h, float("nan"), 1, None) == eb.ECHO_EINVAL
+    assert e.L.echo_run_until(e.h, 1.0, -1, None) == eb.ECHO_EINVAL
