@@ -62,6 +62,31 @@ int cuda_fail(echo_ctx *c, cudaError_t e, const char *where) {
 // flux-sweep tiling: threads per block, transverse width, max tile length
 constexpr int FLUX_NT = 128, FLUX_CMAX = 512;
 
+// Length CZ of the z-chunks of a plane-marching kernel (k_uct2, k_bupd): tiles x chunks blocks run in waves of
+// `slots` resident blocks, and every chunk pays about `fill` planes of pipeline fill (window prologue, first copies).
+// Picks the chunk count with the best  (blocks / (waves * slots)) * CZ / (CZ + fill); at 256^3 this is 6 chunks of 43
+// planes for k_uct2 (3072 blocks = 6.9 waves of 444) instead of 3 of 86 (3.5 waves): 1.15 -> 1.08 ms.
+int pick_chunk_planes(int tiles, int nz, int slots, int fill) {
+    int best_cz = nz;
+    double best = -1.0;
+    for (int nchunk = 1; nchunk <= std::max(1, nz / 8); ++nchunk) {
+        const int cz = (nz + nchunk - 1) / nchunk;
+        const long blocks = (long)tiles * ((nz + cz - 1) / cz);
+        const long waves = (blocks + slots - 1) / slots;
+        const double eff = (double)blocks / (double)(waves * slots) * cz / (double)(cz + fill);
+        if (eff > best * 1.0005) { best = eff; best_cz = cz; }
+    }
+    return best_cz;
+}
+template <typename K>
+int resident_slots(K kernel, int threads) {
+    int per_sm = 0, sms = 0, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0);
+    return std::max(1, per_sm) * std::max(1, sms);
+}
+
 enum { KC_PRIM = 0, KC_FLUX = 1, KC_UCT = 4, KC_UPDATE = 5, KC_CTRL = 6, KC_OTHER = 7 };
 
 size_t next_event(echo_ctx *c) {
@@ -206,13 +231,12 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
     if (set_dt) {   // stage 1 of a step: dt must exist before any update (S9)
         KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
     }
-    {   // plane-marching UCT: 16 x 8 tiles of (x, y), chunks of planes along z sized for >= ~8 blocks per SM
+    {   // plane-marching UCT: 16 x 8 tiles of (x, y), chunks of planes along z sized by pick_chunk_planes
         // (splitting it into an x/y kernel and a z kernel to shed the z-window registers was measured: 1.28 ms
         // against 1.21 ms for the single kernel at 256^3, so the single kernel stays)
         const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
-        int nchunk = (148 * 8 + tiles - 1) / tiles;
-        nchunk = std::max(1, std::min(nchunk, (g.n[2] + 15) / 16));
-        const int CZ = (g.n[2] + nchunk - 1) / nchunk;
+        static const int slots = resident_slots(k_uct2<false>, UCT_NT);
+        const int CZ = pick_chunk_planes(tiles, g.n[2], slots, 3);
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
         if (g.rec == 2) KL(KC_UCT, "k_uct2", k_uct2<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
         else KL(KC_UCT, "k_uct2", k_uct2<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
@@ -247,9 +271,8 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
                                                                               st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
     } else {   // staggered B only: plane-marching curl + update
         const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
-        int nchunk = (148 * 16 + tiles - 1) / tiles;
-        nchunk = std::max(1, std::min(nchunk, (g.n[2] + 15) / 16));
-        const int CZ = (g.n[2] + nchunk - 1) / nchunk;
+        static const int slots = resident_slots(k_bupd, UCT_NT);
+        const int CZ = pick_chunk_planes(tiles, g.n[2], slots, 2);
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
         KL(KC_UPDATE, "k_bupd", k_bupd<<<grid, UCT_NT, 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], up, ctx->ctrl, CZ));
     }
