@@ -65,7 +65,7 @@ __global__ void k_c2p_stats_reset(Ctrl *c) {
 struct PrimUpd { double *uout[8]; const double *bin[3]; };
 
 template <bool STATS, bool UPD, bool UCT = true>
-__global__ void __launch_bounds__(256) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu) {
+__global__ void __launch_bounds__(256, 5) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
