@@ -300,3 +300,108 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const
 }
 
 }  // namespace echo
+
+// ------------------------------------------------------------------ point 1 inside echo_step (UCT = YES)
+// k_prim_march: INT of the staggered B + con2prim (O1, O2) with the data movement of k_bupd: a 16 x 8 tile
+// of (x, y) marches along z; B_x with its x-halo and B_y with its y-halo of plane k+1 arrive by cp.async while plane
+// k is inverted, B_z lives in a 6-plane register window, the conserved fields (and, UPD, the stage-1 rhs) of plane
+// k+1 are loaded into registers one round early.  The Newton iterations of one plane thus overlap the memory
+// latency of the next, which the thread-per-cell k_prim (kept for the STATS passes and UCT = NO) cannot do.
+// Same arithmetic on the same operands as k_prim: bit-identical results.
+namespace echo {
+
+template <bool UPD>
+__global__ void __launch_bounds__(UCT_NT) k_prim_march(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu, int CZ) {
+    __shared__ double sBX[2][BU_XE];       // B_x, x offsets -3 .. TX+1
+    __shared__ double sBY[2][BU_YE];       // B_y, y offsets -3 .. TY+1
+    const int tid = threadIdx.x;
+    const int tx = tid % UCT_TX, ty = tid / UCT_TX;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int x0 = blockIdx.x * UCT_TX, y0 = blockIdx.y * UCT_TY, z0 = blockIdx.z * CZ;
+    const int CZv = min(CZ, nz - z0);
+    const int sy = g.s[1], sz = g.s[2];
+    const double dt = UPD ? ctrl->dt : 0.0;
+
+    int oXE[2], oYE[2];
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int e = tid + UCT_NT * it;
+        oXE[it] = (e < BU_XE) ? wrapi(x0 - 3 + e % UCT_XRW, nx) + sy * wrapi(y0 + e / UCT_XRW, ny) : -1;
+        oYE[it] = (e < BU_YE) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 - 3 + e / UCT_TX, ny) : -1;
+    }
+    auto issue_plane = [&](int k, int slot) {
+        const int pz = sz * wrapi(k, nz);
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = tid + UCT_NT * it;
+            if (oXE[it] >= 0) cp_async8(&sBX[slot][e], st.Bf[0] + (pz + oXE[it]));
+            if (oYE[it] >= 0) cp_async8(&sBY[slot][e], st.Bf[1] + (pz + oYE[it]));
+        }
+        cp_async_commit();
+    };
+    const bool cellok = (x0 + tx < nx) && (y0 + ty < ny);
+    const int ccol = min(x0 + tx, nx - 1) + sy * min(y0 + ty, ny - 1);
+    const bool inxy = (x0 + tx) >= g.lo[0] && (x0 + tx) < g.hi[0] && (y0 + ty) >= g.lo[1] && (y0 + ty) < g.hi[1];
+
+    issue_plane(z0, 0);
+    double wz[6];                          // B_z of planes k-3 .. k+2
+#pragma unroll
+    for (int m = 0; m < 6; ++m) wz[m] = __ldg(st.Bf[2] + (sz * wrapi(z0 - 3 + m, nz) + ccol));
+    double un[5], rn[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        un[v] = __ldg(st.U[v] + (sz * z0 + ccol));
+        rn[v] = UPD ? __ldg(st.R[v] + (sz * z0 + ccol)) : 0.0;
+    }
+
+    for (int r = 0; r < CZv; ++r) {
+        const int k = z0 + r;
+        cp_async_wait_all();
+        __syncthreads();
+        const bool more = (r + 1 < CZv);
+        double nwz = 0.0, nu[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, nr[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        if (more) {
+            issue_plane(k + 1, (r + 1) & 1);
+            nwz = __ldg(st.Bf[2] + (sz * wrapi(k + 3, nz) + ccol));
+            const int o = sz * (k + 1) + ccol;
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                nu[v] = __ldg(st.U[v] + o);
+                if (UPD) nr[v] = __ldg(st.R[v] + o);
+            }
+        }
+        if (cellok) {
+            const int ps = r & 1;
+            const double *px = &sBX[ps][ty * UCT_XRW + tx], *py = &sBY[ps][ty * UCT_TX + tx];
+            constexpr int S = UCT_TX;
+            double B[3];
+            B[0] = int_ho(g.ho, px[0], px[1], px[2], px[3], px[4], px[5]);
+            B[1] = int_ho(g.ho, py[0], py[S], py[2 * S], py[3 * S], py[4 * S], py[5 * S]);
+            B[2] = int_ho(g.ho, wz[0], wz[1], wz[2], wz[3], wz[4], wz[5]);
+            const int o = sz * k + ccol;
+            double u[5];
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                u[v] = un[v];
+                if (UPD) {
+                    u[v] = u[v] + dt * rn[v];
+                    pu.uout[v][o] = u[v];
+                }
+            }
+            double q[5];
+            const int it = con2prim(gam, u, B, q);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) st.P[v][o] = q[v];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) st.Bc[d][o] = B[d];
+            if (it < 0 && inxy && k >= g.lo[2] && k < g.hi[2]) atomicAdd(&ctrl->c2p_fail_total, 1ull);
+        }
+#pragma unroll
+        for (int m = 0; m < 5; ++m) wz[m] = wz[m + 1];
+        wz[5] = nwz;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) { un[v] = nu[v]; rn[v] = nr[v]; }
+    }
+}
+
+}  // namespace echo
