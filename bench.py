@@ -167,7 +167,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": "fp64_cell_updates_per_sec", "value": rate, "unit": "cell-updates/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "cpa_wave_%s_%d^3_oracle_sample" % (args.direction, n), "gamma": GAMMA, "cfl": CFL},
+            # the arm's own workload (same name as the echo arm prints); each step advances a bounded sample of it
+            "config": {"workload": "cpa_wave_%s_%d^3" % (args.direction, args.n), "gamma": GAMMA, "cfl": CFL,
+                       "scheme": "MP5+HLL+UCT+DER6/INT6+SSPRK3 (UCT=HO=YES)", "sample": sample},
             "cpu_baseline": {"value": rate, "unit": "cell-updates/s", "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": rate, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
