@@ -205,6 +205,11 @@ int launch_sweeps(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan
             KL(KC_PRIM, "k_prim_cc", k_prim<false, true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
         else
             KL(KC_PRIM, "k_prim_cc", k_prim<false, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+    } else if (g.n[2] < 8) {   // a thin grid (2.5-D runs): nothing to march along, the thread-per-cell kernel is faster
+        if (pl && pl->prim_upd)
+            KL(KC_PRIM, "k_prim", k_prim<false, true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+        else
+            KL(KC_PRIM, "k_prim", k_prim<false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
     } else {   // plane-marching INT + con2prim (k_prim_march), tiles and z-chunks as for k_bupd
         const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
         static const int slots = resident_slots(k_prim_march<true>, UCT_NT);

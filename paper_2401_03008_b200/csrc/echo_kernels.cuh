@@ -368,6 +368,15 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
     if (i < g.n[0] && j < g.n[1]) {
         const int c = i + g.s[1] * j + g.s[2] * k;
         constexpr int NC = UCT ? 5 : 8;
+        double ub[NC], uc[NC], rr[NC];             // MODE 1: what the update needs, loaded ahead of the face arithmetic
+        if (MODE == 1) {
+#pragma unroll
+            for (int v = 0; v < NC; ++v) {
+                ub[v] = __ldg(up.base[v] + c);
+                uc[v] = up.cur[v][c];
+                rr[v] = __ldg((v < 5 ? st.R[v] : st.E[v - 5]) + c);
+            }
+        }
         const double *rec[8] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], UCT ? st.Bc[t1] : st.Bc[0],
                                 UCT ? st.Bc[t2] : st.Bc[1], st.Bc[2]};
         constexpr int slot[8] = {0, 1, 2, 3, 4, UCT ? 5 + t1 : 5, UCT ? 5 + t2 : 6, 7};
@@ -394,9 +403,7 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
             const double dt = ctrl->dt;
             if (ctrl->active) {
 #pragma unroll
-                for (int v = 0; v < NC; ++v)
-                    up.out[v][c] = up.c0 * __ldg(up.base[v] + c) +
-                                   up.c1 * (up.cur[v][c] + dt * __ldg((v < 5 ? st.R[v] : st.E[v - 5]) + c));
+                for (int v = 0; v < NC; ++v) up.out[v][c] = up.c0 * ub[v] + up.c1 * (uc[v] + dt * rr[v]);
             }
         } else if (D == 0) {
 #pragma unroll
