@@ -60,7 +60,9 @@ int cuda_fail(echo_ctx *c, cudaError_t e, const char *where) {
     } while (0)
 
 // flux-sweep tiling: threads per block, transverse width, max tile length
-constexpr int FLUX_NT = 128, FLUX_CMAX = 512;
+// threads per block of the y/z sweeps and of the x-sweep (x marches 32 / 16 rows per round with 128 / 64 threads: a
+// 256-cell row costs 10 rounds of 32 or 18 of 16, i.e. 320 or 288 row slots for its 261 faces: 0.74 -> 0.71 ms)
+constexpr int FLUX_NT = 128, FLUX_NT_X = 64, FLUX_CMAX = 512;
 
 // Length CZ of the z-chunks of a plane-marching kernel (k_uct2, k_bupd): tiles x chunks blocks run in waves of
 // `slots` resident blocks, and every chunk pays about `fill` planes of pipeline fill (window prologue, first copies).
@@ -135,9 +137,9 @@ Stage make_stage(const echo_ctx *c, int which) {
 }
 
 // fuse: 0 = plain operator (rhs written), 1 = the z-sweep applies the RK combination of the 5 cell fields
-template <int D, int MODE>
-int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu) {
-    constexpr int NT = FLUX_NT, T = (D == 0) ? 4 : 16;
+template <int D, int MODE, int NT>
+int launch_flux_nt(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu) {
+    constexpr int T = (D == 0) ? 4 : 16;
     constexpr int TD = (D == 0) ? 1 : 0, OD = 3 - D - TD;
     const Grid &g = ctx->g;
     if (g.n[D] == 1) {   // a one-cell axis: no stencil work left, only the face quantities (k_flux_flat)
@@ -184,6 +186,13 @@ int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu
     else
         KL(KC_FLUX + D, "k_flux", k_flux<D, NT, MODE, false><<<grid, NT, 0, ctx->stream>>>(g, st, C, ctx->gamma, ctx->gg, ctx->ctrl, want_amax, fu));
     return ECHO_OK;
+}
+
+template <int D, int MODE>
+int launch_flux(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd &fu) {
+    // the x-sweep of the MP5 scheme runs 64-thread blocks; with the cheap linear REC the larger block is the faster one
+    if (D == 0 && ctx->g.rec != 2) return launch_flux_nt<D, MODE, (D == 0) ? FLUX_NT_X : FLUX_NT>(ctx, st, want_amax, fu);
+    return launch_flux_nt<D, MODE, FLUX_NT>(ctx, st, want_amax, fu);
 }
 
 // RK bookkeeping of one stage inside echo_step: which buffers hold what

@@ -193,7 +193,7 @@ struct FluxUpd { const double *base[8]; const double *cur[8]; double *out[8]; do
 // quantities for UCT.  The inputs are the k_prim copies st.Bc, not the evolved st.Bf: the fused RK update of
 // MODE 1 overwrites the evolved B while wrapped rows of it are still to be read.  Compile-time branches only: the UCT = true instantiations are the kernel described above.
 template <int D, int NT, int MODE, bool HO, bool UCT = true, int REC = 5>
-__global__ void __launch_bounds__(NT, 4) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
+__global__ void __launch_bounds__(NT, 512 / NT) k_flux(Grid g, Stage st, int C, double gam, double gg, Ctrl *ctrl,
                                              int want_amax, FluxUpd up) {
     constexpr int TD = (D == 0) ? 1 : 0;      // contiguous transverse axis of the tile
     constexpr int OD = 3 - D - TD;            // remaining axis
