@@ -412,7 +412,7 @@ def run_gpu(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch and per CELL from the committed ncu --set full capture
 # (profiles/r1_ncu_full.md: 256^3, RK stage 2), keyed by kernel class; bench.py reports it times the cells of a launch.
-TRAFFIC_PER_CELL = {"k_prim": 206.0, "k_flux_x": 135.4, "k_flux_y": 177.3, "k_flux_z": 258.4, "k_uct": 164.2,
+TRAFFIC_PER_CELL = {"k_prim": 206.0, "k_flux_x": 149.3, "k_flux_y": 177.3, "k_flux_z": 258.4, "k_uct": 164.2,
                     "k_update": 95.8}
 
 
