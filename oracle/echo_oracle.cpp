@@ -27,8 +27,10 @@
 // treated as the other cell-centered variables").
 //
 // Pins (tests/test_oracle_*.py): see the list in DESIGN.md §"Oracle pins".
-// parity unpinned: the MP5 limiter branch on non-smooth data (the paper prints nothing
-// that fixes it; only its invariants are tested).
+// parity unpinned: inside the MP5 limiter branch, the published design constants 1/2 (v^MD), 4/3 (v^LC) and 4
+// (inside d^M4) against nearby values.  The paper prints nothing that fixes them; what IS pinned about the branch
+// (tests/test_oracle_units.py, tests/test_oracle_mp5_advection.py): its bounds and symmetries, monotone advection
+// of a pulse at Courant number 1/(1+alpha), transparency on resolved smooth extrema, the bound v_j + alpha dv.
 
 #include <cmath>
 #include <cstddef>

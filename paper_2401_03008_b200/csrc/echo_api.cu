@@ -254,6 +254,15 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
     {   // plane-marching UCT: 16 x 8 tiles of (x, y), chunks of planes along z sized by pick_chunk_planes
         // (splitting it into an x/y kernel and a z kernel to shed the z-window registers was measured: 1.28 ms
         // against 1.21 ms for the single kernel at 256^3, so the single kernel stays)
+        if (g.n[2] == 1) {   // 2.5-D: the same kernel marching along y (k_uct2_flat)
+            const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
+            static const int fslots = resident_slots(k_uct2_flat<false>, UCT_NT);
+            const int CY = pick_chunk_planes(tx, ty, fslots, 3);
+            dim3 grid(tx, (ty + CY - 1) / CY, 1);
+            if (g.rec == 2) KL(KC_UCT, "k_uct2_flat", k_uct2_flat<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CY));
+            else KL(KC_UCT, "k_uct2_flat", k_uct2_flat<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CY));
+            return ECHO_OK;
+        }
         const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
         static const int slots = resident_slots(k_uct2<false>, UCT_NT);
         const int CZ = pick_chunk_planes(tiles, g.n[2], slots, 3);
@@ -289,6 +298,12 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
     if (with_u) {
         KL(KC_UPDATE, "k_update", k_update<true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], st.R[0], st.R[1],
                                                                               st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
+    } else if (g.n[2] == 1) {   // 2.5-D: curl + update marching along y (k_bupd_flat)
+        const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
+        static const int fslots = resident_slots(k_bupd_flat, UCT_NT);
+        const int CY = pick_chunk_planes(tx, ty, fslots, 2);
+        dim3 grid(tx, (ty + CY - 1) / CY, 1);
+        KL(KC_UPDATE, "k_bupd_flat", k_bupd_flat<<<grid, UCT_NT, 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], up, ctx->ctrl, CY));
     } else {   // staggered B only: plane-marching curl + update
         const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
         static const int slots = resident_slots(k_bupd, UCT_NT);

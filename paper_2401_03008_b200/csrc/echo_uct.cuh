@@ -301,13 +301,250 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const
 
 }  // namespace echo
 
+// ------------------------------------------------------------------ 2.5-D grids (n_z = 1): march along y
+// With one plane there is nothing to march along in z and a block of the kernels above would load one tile, wait
+// for it, compute and exit.  k_uct2_flat / k_bupd_flat run the same arithmetic with the roles of "plane" taken by
+// consecutive (x, y) tiles along y: the tiles of y-tile t+1 arrive by cp.async while tile t is computed.  Through the
+// periodic wrap the six z-stencil values of a cell are all the cell's own value and plane k+1 is plane k, so the
+// z-brackets see six equal values (the generic arithmetic applied to them: bitwise what k_uct2 / k_bupd give on a
+// one-plane grid, and what a thicker grid with z-independent data gives - the dimensional-reduction tests).
+namespace echo {
+
+template <bool LIN = false>
+__global__ void __launch_bounds__(UCT_NT) k_uct2_flat(Grid g, Stage st, int CY) {
+    __shared__ double sXR[2][4][UCT_XR];
+    __shared__ double sYR[2][4][UCT_YR];
+    __shared__ double sAZ[2][2][UCT_AZ];
+    __shared__ double sAX[2][2][UCT_AX];
+    __shared__ double sAY[2][2][UCT_AY];
+
+    const int tid = threadIdx.x;
+    const int tx = tid % UCT_TX, ty = tid / UCT_TX;
+    const int nx = g.n[0], ny = g.n[1];
+    const int ntile = (ny + UCT_TY - 1) / UCT_TY;
+    const int x0 = blockIdx.x * UCT_TX, t0 = blockIdx.y * CY;
+    const int CYv = min(CY, ntile - t0);
+    const int sy = g.s[1];
+
+    // per-thread copy map: wrapped x offset and row of the (at most two) elements per region
+    int xXR[2], xYR[2], xAX[2], xAY[2];
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int e = tid + UCT_NT * it;
+        xXR[it] = (e < UCT_XR) ? wrapi(x0 - 2 + e % UCT_XRW, nx) : -1;
+        xYR[it] = (e < UCT_YR) ? wrapi(x0 + e % UCT_TX, nx) : -1;
+        xAX[it] = (e < UCT_AX) ? wrapi(x0 + e % UCT_TX, nx) : -1;
+        xAY[it] = (e < UCT_AZ) ? wrapi(x0 + e % UCT_AYW, nx) : -1;      // AY (8 rows) and AZ (9 rows) share it
+    }
+    const double *fXR[4] = {st.vb[1][1], st.Bf[1], st.vb[2][0], st.Bf[2]};
+    const double *fYR[4] = {st.vb[0][0], st.Bf[0], st.vb[2][1], st.Bf[2]};
+    const double *fZW[4] = {st.vb[0][1], st.Bf[0], st.vb[1][0], st.Bf[1]};
+
+    auto issue_tile = [&](int y0, int slot) {
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = tid + UCT_NT * it;
+            if (xXR[it] >= 0) {
+                const int o = xXR[it] + sy * wrapi(y0 + e / UCT_XRW, ny);
+#pragma unroll
+                for (int f = 0; f < 4; ++f) cp_async8(&sXR[slot][f][e], fXR[f] + o);
+            }
+            if (xYR[it] >= 0) {
+                const int o = xYR[it] + sy * wrapi(y0 - 2 + e / UCT_TX, ny);
+#pragma unroll
+                for (int f = 0; f < 4; ++f) cp_async8(&sYR[slot][f][e], fYR[f] + o);
+            }
+            if (xAX[it] >= 0) {
+                const int o = xAX[it] + sy * wrapi(y0 + e / UCT_TX, ny);
+                cp_async8(&sAX[slot][0][e], st.ap[0] + o);
+                cp_async8(&sAX[slot][1][e], st.am[0] + o);
+            }
+            if (xAY[it] >= 0) {
+                const int o = xAY[it] + sy * wrapi(y0 + e / UCT_AYW, ny);
+                if (e < UCT_AY) {
+                    cp_async8(&sAY[slot][0][e], st.ap[1] + o);
+                    cp_async8(&sAY[slot][1][e], st.am[1] + o);
+                }
+                cp_async8(&sAZ[slot][0][e], st.ap[2] + o);
+                cp_async8(&sAZ[slot][1][e], st.am[2] + o);
+            }
+        }
+        cp_async_commit();
+    };
+    const bool xok = (x0 + tx) < nx;
+    const int cx = min(x0 + tx, nx - 1);
+    auto cell = [&](int t) { return cx + sy * min(t * UCT_TY + ty, ny - 1); };
+
+    issue_tile(t0 * UCT_TY, 0);
+    double zc[4];
+#pragma unroll
+    for (int f = 0; f < 4; ++f) zc[f] = __ldg(fZW[f] + cell(t0));
+
+    for (int r = 0; r < CYv; ++r) {
+        const int t = t0 + r;
+        cp_async_wait_all();
+        __syncthreads();
+        double zn[4] = {0.0, 0.0, 0.0, 0.0};
+        if (r + 1 < CYv) {
+            issue_tile((t + 1) * UCT_TY, (r + 1) & 1);
+#pragma unroll
+            for (int f = 0; f < 4; ++f) zn[f] = __ldg(fZW[f] + cell(t + 1));
+        }
+        if (xok && (t * UCT_TY + ty) < ny) {
+            const int ps = r & 1;
+            const int iax = ty * UCT_TX + tx, iay = ty * UCT_AYW + tx;
+            const double axp = sAX[ps][0][iax], axm = sAX[ps][1][iax];
+            const double ayp = sAY[ps][0][iay], aym = sAY[ps][1][iay];
+            const double azp = sAZ[ps][0][iay], azm = sAZ[ps][1][iay];
+            auto bracket = [&](const double *p, const double *q, int S, double ap, double am) {
+                double vL, vR, BL, BR;
+                if (LIN) {
+                    tvd2_pair(p[S], p[2 * S], p[3 * S], p[4 * S], vL, vR);
+                    tvd2_pair(q[S], q[2 * S], q[3 * S], q[4 * S], BL, BR);
+                    return uct_hll(ap, am, vL, vR, BL, BR);
+                }
+                const unsigned nv = mp5_pair_fast(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+                const unsigned nb = mp5_pair_fast(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+                if (nv | nb) {
+                    mp5_pair_fix(nv, p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+                    mp5_pair_fix(nb, q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+                }
+                return uct_hll(ap, am, vL, vR, BL, BR);
+            };
+            auto along_x = [&](int f, double ap, double am) {
+                const double *p = &sXR[ps][f][ty * UCT_XRW + tx];
+                return bracket(p, p + UCT_XR, 1, ap, am);
+            };
+            auto along_y = [&](int f, double ap, double am) {
+                const double *p = &sYR[ps][f][ty * UCT_TX + tx];
+                return bracket(p, p + UCT_YR, UCT_TX, ap, am);
+            };
+            auto along_z = [&](int f, double ap, double am) {      // six equal values: the cell's own
+                const double a = zc[f], b = zc[f + 1];
+                const double pa[6] = {a, a, a, a, a, a}, qb[6] = {b, b, b, b, b, b};
+                return bracket(pa, qb, 1, ap, am);
+            };
+            // E_z: i = x, j = y
+            const double ez = -along_x(0, dmax(axp, sAX[ps][0][iax + UCT_TX]), dmax(axm, sAX[ps][1][iax + UCT_TX])) +
+                              along_y(0, dmax(ayp, sAY[ps][0][iay + 1]), dmax(aym, sAY[ps][1][iay + 1]));
+            // E_y: i = z, j = x   (plane k+1 is plane k)
+            const double ey = -along_z(0, dmax(azp, sAZ[ps][0][iay + 1]), dmax(azm, sAZ[ps][1][iay + 1])) +
+                              along_x(2, dmax(axp, axp), dmax(axm, axm));
+            // E_x: i = y, j = z
+            const double ex = -along_y(2, dmax(ayp, ayp), dmax(aym, aym)) +
+                              along_z(2, dmax(azp, sAZ[ps][0][iay + UCT_AYW]), dmax(azm, sAZ[ps][1][iay + UCT_AYW]));
+            const int o = cell(t);
+            st.E[0][o] = ex;
+            st.E[1][o] = ey;
+            st.E[2][o] = ez;
+        }
+#pragma unroll
+        for (int f = 0; f < 4; ++f) zc[f] = zn[f];
+    }
+}
+
+__global__ void __launch_bounds__(UCT_NT) k_bupd_flat(Grid g, const double *E0, const double *E1, const double *E2, Update up,
+                                                      const Ctrl *ctrl, int CY) {
+    __shared__ double sXE[2][2][BU_XE];    // E_z, E_y (differenced along x)
+    __shared__ double sYE[2][2][BU_YE];    // E_z, E_x (differenced along y)
+    const int tid = threadIdx.x;
+    const int tx = tid % UCT_TX, ty = tid / UCT_TX;
+    const int nx = g.n[0], ny = g.n[1];
+    const int ntile = (ny + UCT_TY - 1) / UCT_TY;
+    const int x0 = blockIdx.x * UCT_TX, t0 = blockIdx.y * CY;
+    const int CYv = min(CY, ntile - t0);
+    const int sy = g.s[1];
+    const double dt = ctrl->dt;
+    const int active = ctrl->active;
+
+    int xXE[2], xYE[2];
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int e = tid + UCT_NT * it;
+        xXE[it] = (e < BU_XE) ? wrapi(x0 - 3 + e % UCT_XRW, nx) : -1;
+        xYE[it] = (e < BU_YE) ? wrapi(x0 + e % UCT_TX, nx) : -1;
+    }
+    auto issue_tile = [&](int y0, int slot) {
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int e = tid + UCT_NT * it;
+            if (xXE[it] >= 0) {
+                const int o = xXE[it] + sy * wrapi(y0 + e / UCT_XRW, ny);
+                cp_async8(&sXE[slot][0][e], E2 + o);
+                cp_async8(&sXE[slot][1][e], E1 + o);
+            }
+            if (xYE[it] >= 0) {
+                const int o = xYE[it] + sy * wrapi(y0 - 3 + e / UCT_TX, ny);
+                cp_async8(&sYE[slot][0][e], E2 + o);
+                cp_async8(&sYE[slot][1][e], E0 + o);
+            }
+        }
+        cp_async_commit();
+    };
+    const bool xok = (x0 + tx) < nx;
+    const int cx = min(x0 + tx, nx - 1);
+    auto cell = [&](int t) { return cx + sy * min(t * UCT_TY + ty, ny - 1); };
+
+    issue_tile(t0 * UCT_TY, 0);
+    double ec[2], bc[3], bb[3];            // E_y, E_x of the cell (its whole z-stencil), cur and base B
+    {
+        const int o = cell(t0);
+        ec[0] = __ldg(E1 + o);
+        ec[1] = __ldg(E0 + o);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { bc[d] = up.cur[5 + d][o]; bb[d] = __ldg(up.base[5 + d] + o); }
+    }
+    for (int r = 0; r < CYv; ++r) {
+        const int t = t0 + r;
+        cp_async_wait_all();
+        __syncthreads();
+        double nec[2] = {0.0, 0.0}, nbc[3] = {0.0, 0.0, 0.0}, nbb[3] = {0.0, 0.0, 0.0};
+        if (r + 1 < CYv) {
+            issue_tile((t + 1) * UCT_TY, (r + 1) & 1);
+            const int o = cell(t + 1);
+            nec[0] = __ldg(E1 + o);
+            nec[1] = __ldg(E0 + o);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { nbc[d] = up.cur[5 + d][o]; nbb[d] = __ldg(up.base[5 + d] + o); }
+        }
+        if (xok && (t * UCT_TY + ty) < ny && active) {
+            const int ps = r & 1;
+            const double *pz_x = &sXE[ps][0][ty * UCT_XRW + tx], *py_x = pz_x + BU_XE;
+            const double *pz_y = &sYE[ps][0][ty * UCT_TX + tx], *px_y = pz_y + BU_YE;
+            constexpr int S = UCT_TX;
+            const double dxEz = der_diff_ho(g.ho, pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
+            const double dxEy = der_diff_ho(g.ho, py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
+            const double dyEz = der_diff_ho(g.ho, pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
+            const double dyEx = der_diff_ho(g.ho, px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
+            const double dzEy = der_diff_ho(g.ho, ec[0], ec[0], ec[0], ec[0], ec[0], ec[0]);
+            const double dzEx = der_diff_ho(g.ho, ec[1], ec[1], ec[1], ec[1], ec[1], ec[1]);
+            double rb[3];
+            rb[0] = -(g.rh[1] * dyEz - g.rh[2] * dzEy);
+            rb[1] = -(g.rh[2] * dzEx - g.rh[0] * dxEz);
+            rb[2] = -(g.rh[0] * dxEy - g.rh[1] * dyEx);
+            const int o = cell(t);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const double adv = bc[d] + dt * rb[d];
+                up.out[5 + d][o] = (up.c0 == 0.0) ? adv : up.c0 * bb[d] + up.c1 * adv;
+            }
+        }
+        ec[0] = nec[0]; ec[1] = nec[1];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { bc[d] = nbc[d]; bb[d] = nbb[d]; }
+    }
+}
+
+}  // namespace echo
+
 // ------------------------------------------------------------------ point 1 inside echo_step (UCT = YES)
 // k_prim_march: INT of the staggered B + con2prim (O1, O2) with the data movement of k_bupd: a 16 x 8 tile
 // of (x, y) marches along z; B_x with its x-halo and B_y with its y-halo of plane k+1 arrive by cp.async while plane
 // k is inverted, B_z lives in a 6-plane register window, the conserved fields (and, UPD, the stage-1 rhs) of plane
 // k+1 are loaded into registers one round early.  The Newton iterations of one plane thus overlap the memory
 // latency of the next, which the thread-per-cell k_prim (kept for the STATS passes and UCT = NO) cannot do.
-// Same arithmetic on the same operands as k_prim: bit-identical results.
+// Same formulas on the same operands as k_prim; the compiler schedules and contracts them differently in the two
+// kernels, so the results agree to round-off (a few ulp), not bit for bit.
 namespace echo {
 
 template <bool UPD>

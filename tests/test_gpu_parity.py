@@ -307,6 +307,38 @@ def test_turbulence_2d_paper_setup(torch, eb, ob):
     assert dg["max_div_b"] <= 1e-12 * w["B0"] * 64 * 50
 
 
+@pytest.mark.parametrize("order", [(5, 3), (2, 2)])
+def test_flat_kernels_equal_the_plane_marching_ones_bitwise(torch, eb, ob, order):
+    """n_z = 1 runs through k_uct2_flat / k_bupd_flat / k_flux_flat (tiles marching along y); the same 2-D data
+    stacked on 4 planes runs through the plane-marching k_uct2 / k_bupd and the generic z-sweep.  Same arithmetic per
+    cell, so the two must agree BIT FOR BIT; 70 x 83 is ragged in both tile directions and long enough along y for
+    several chunks of tiles per block, the last step is clipped.  On 8 planes INT + con2prim run in k_prim_march
+    instead of k_prim (another instruction schedule of the same formulas): agreement to round-off."""
+    nx, ny = 70, 83
+    w = inputs.turbulence_2d(nx, ny)
+    bo = ob.faces_from_potential(w["ax"], w["ay"], w["az"])
+    w["bxf"], w["byf"], w["bzf"] = [b + w["b0"][d] for d, b in enumerate(bo)]
+    runs = {}
+    for nz in (1, 4, 8):
+        e = eb.Echo(nx, ny, nz, G, 0.3, ho=(order == (5, 3)), rec=order[0], rk=order[1])
+        e.set_primitives(*[dev(torch, np.array(np.broadcast_to(w[k], (nz, ny, nx)))) for k in SETK])
+        e.step(4, 3.4 * 0.3 / 83 / 0.95)
+        d = e.diagnostics()
+        assert d["c2p_failures"] == 0 and d["steps"] in (3, 4)
+        runs[nz] = (d, {**e.get_primitives(), **e.get_conserved()})
+    d1, q1 = runs[1]
+    for nz, exact in ((4, True), (8, False)):
+        d, q = runs[nz]
+        assert d["steps"] == d1["steps"] and d["t"] == pytest.approx(d1["t"], rel=1e-14)
+        for k in q1:
+            a, b = q[k].cpu().numpy(), q1[k].cpu().numpy()
+            b = np.broadcast_to(b, a.shape)
+            if exact:
+                assert d["t"] == d1["t"] and np.array_equal(a, b), (nz, k)
+            else:
+                assert np.abs(a - b).max() <= 1e-12 * max(1.0, np.abs(b).max()), (nz, k)
+
+
 def test_async_host_readback_two_streams(torch, eb, ob):
     """echo_get_primitives_host_async + echo_synchronize on two handles bound to two streams (the pipelined
     end-to-end path of bench.py) return exactly what the synchronous call returns."""
