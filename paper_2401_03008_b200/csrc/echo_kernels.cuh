@@ -178,6 +178,7 @@ __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) 
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const double *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -263,14 +264,24 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_flux(Grid g, Stage st, int C, 
         double rold[NC], ucur[NC], ubase[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) rold[c] = 0.0;
+        constexpr bool LATE = (MODE == 1) && !UCT;   // 24 operands do not fit beside the face arithmetic: prefetch now, load at (3b)
         if (do2) {
-            if (D != 0) {
+            if (LATE) {
 #pragma unroll
-                for (int c = 0; c < NC; ++c) rold[c] = __ldg((c < 5 ? st.R[c] : st.E[c - 5]) + o2);
-            }
-            if (MODE == 1) {
+                for (int c = 0; c < NC; ++c) {
+                    prefetch_l2((c < 5 ? st.R[c] : st.E[c - 5]) + o2);
+                    prefetch_l2(up.cur[c] + o2);
+                    prefetch_l2(up.base[c] + o2);
+                }
+            } else {
+                if (D != 0) {
 #pragma unroll
-                for (int c = 0; c < NC; ++c) { ucur[c] = __ldg(up.cur[c] + o2); ubase[c] = __ldg(up.base[c] + o2); }
+                    for (int c = 0; c < NC; ++c) rold[c] = __ldg((c < 5 ? st.R[c] : st.E[c - 5]) + o2);
+                }
+                if (MODE == 1) {
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) { ucur[c] = __ldg(up.cur[c] + o2); ubase[c] = __ldg(up.base[c] + o2); }
+                }
             }
         }
 
@@ -324,6 +335,14 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_flux(Grid g, Stage st, int C, 
 #pragma unroll
             for (int k = 0; k < 6; ++k) { sl[k] = r0 * FR; r0 = (r0 + 1 == RL) ? 0 : r0 + 1; }
             const double *Fb = sF + b * SB;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                if (LATE) {
+                    rold[c] = __ldg((c < 5 ? st.R[c] : st.E[c - 5]) + o2);
+                    ucur[c] = __ldg(up.cur[c] + o2);
+                    ubase[c] = __ldg(up.base[c] + o2);
+                }
+            }
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const double *F = Fb + c * FV;
