@@ -388,12 +388,12 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
         const int c = i + g.s[1] * j + g.s[2] * k;
         constexpr int NC = UCT ? 5 : 8;
         double ub[NC], uc[NC], rr[NC];             // MODE 1: what the update needs, loaded ahead of the face arithmetic
-        if (MODE == 1) {
+        if (MODE == 1) {   // prefetched now (no registers), loaded after the face arithmetic
 #pragma unroll
             for (int v = 0; v < NC; ++v) {
-                ub[v] = __ldg(up.base[v] + c);
-                uc[v] = up.cur[v][c];
-                rr[v] = __ldg((v < 5 ? st.R[v] : st.E[v - 5]) + c);
+                prefetch_l2(up.base[v] + c);
+                prefetch_l2(up.cur[v] + c);
+                prefetch_l2((v < 5 ? st.R[v] : st.E[v - 5]) + c);
             }
         }
         const double *rec[8] = {st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], UCT ? st.Bc[t1] : st.Bc[0],
@@ -421,6 +421,12 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
         if (MODE == 1) {
             const double dt = ctrl->dt;
             if (ctrl->active) {
+#pragma unroll
+                for (int v = 0; v < NC; ++v) {
+                    ub[v] = __ldg(up.base[v] + c);
+                    uc[v] = up.cur[v][c];
+                    rr[v] = __ldg((v < 5 ? st.R[v] : st.E[v - 5]) + c);
+                }
 #pragma unroll
                 for (int v = 0; v < NC; ++v) up.out[v][c] = up.c0 * ub[v] + up.c1 * (uc[v] + dt * rr[v]);
             }
