@@ -255,12 +255,12 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident throughput: W warm-up steps, then EXACTLY K timed steps
+    # ---- device-resident throughput: W warm-up steps, then EXACTLY K timed steps, per-kernel timers OFF
     sampler = ClockSampler(local)       # started before the warm-up so that nvidia-smi is already polling
     sampler.start()                     # when the timed region begins (samples cover warm-up + timed steps)
     stepper(W)
     barrier()
-    e.timing(True)                      # per-kernel CUDA-event brackets on the launching stream
+    e.timing(False)                     # also clears the launch counters
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
@@ -269,11 +269,23 @@ def run_gpu(args):
     barrier()
     clocks = sampler.stop()
     ms = ev0.elapsed_time(ev1)
+    nlaunch = sum(cnt for _, cnt in e.get_timing().values())       # kernels launched inside the timed region
+    value, ms_max = whole_job_rate(N, K, ms, "cuda", world)
+    # ---- second pass, only for the per-kernel split: the same steps with a CUDA-event pair around every launch
+    # (the brackets cost a little, so this pass never feeds `value`); one untimed step first grows the event pool
+    Kk = min(K, args.kernel_steps)
+    e.timing(True)
+    stepper(1)
+    e.timing(True)
+    ev0.record()
+    stepper(Kk)
+    ev1.record()
+    barrier()
+    ms_kpass = ev0.elapsed_time(ev1)
     ktimes = e.get_timing()
     e.timing(False)
     d = e.diagnostics()
-    assert d["rc"] == 0 and d["steps"] == W + K, d
-    value, ms_max = whole_job_rate(N, K, ms, "cuda", world)
+    assert d["rc"] == 0 and d["steps"] == W + K + 1 + Kk, d
 
     # ---- end to end through the C ABI with HOST buffers: every step uploads its inputs from pinned host
     # memory (echo_set_primitives_host), advances one RK3 step and reads the primitives back to the host
@@ -340,11 +352,11 @@ def run_gpu(args):
     for name, (tot, cnt) in ktimes.items():
         if cnt and name in ALGO:
             avg = tot / cnt
-            kernels[name] = {"ms_avg": avg, "launches": cnt, "share": tot / ms,
+            kernels[name] = {"ms_avg": avg, "launches": cnt, "share": tot / ms_kpass,
                              "tflops": ALGO[name]["flop"] * N / (avg * 1e-3) * 1e-12,
                              "gbs": 8 * ALGO[name]["dbl"] * N / (avg * 1e-3) * 1e-9}
         elif cnt:
-            kernels[name] = {"ms_avg": tot / cnt, "launches": cnt, "share": tot / ms}
+            kernels[name] = {"ms_avg": tot / cnt, "launches": cnt, "share": tot / ms_kpass}
     dom = max((k for k in kernels if k in ALGO), key=lambda k: kernels[k]["share"] * 1.0)
     kd = kernels[dom]
     t_alu = ALGO[dom]["flop"] / (fp64_sust * 1e12)
@@ -354,8 +366,8 @@ def run_gpu(args):
                 "frac": kd["tflops"] / fp64_sust}
     else:
         roof = {"bound": "hbm", "achieved": kd["gbs"], "peak": hbm_peak, "unit": "GB/s", "frac": kd["gbs"] / hbm_peak}
-    roof.update(kernel=dom, traffic=(TRAFFIC_PER_CELL[dom] * N if dom in TRAFFIC_PER_CELL and args.scheme == "uct-ho" else None),
-                traffic_source="ncu dram bytes per cell of profiles/r1_ncu_full.md (256^3, stage 2) x cells of this launch", peak_source=("FP64 DFMA micro-benchmark run by this bench "
+    traffic, traffic_source = measured_traffic(dom, N, args)
+    roof.update(kernel=dom, traffic=traffic, traffic_source=traffic_source, peak_source=("FP64 DFMA micro-benchmark run by this bench "
                 "(sustained; burst %.1f)" % fp64_burst) if roof["bound"] == "alu" else "MEASURED_PEAKS.json (%s)" % peak_kind,
                 algorithmic_flop_per_cell=ALGO[dom]["flop"], algorithmic_bytes_per_cell=8 * ALGO[dom]["dbl"],
                 ms_per_launch=kd["ms_avg"], cells_per_launch=N)
@@ -373,7 +385,6 @@ def run_gpu(args):
         vs_baseline = value / PAPER_512_PER_NODE[args.scheme]
         baseline_note = ("paper: %.3g cell-updates/s on one LEONARDO node (4 x A100 64 GB) for this workload and scheme "
                          "(BASELINE.md section 1); this run: %d x B200" % (PAPER_512_PER_NODE[args.scheme], world))
-    nlaunch = sum(cnt for _, cnt in ktimes.values())
     line = {"metric": "fp64_cell_updates_per_sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": vs_baseline, "dtype": "f64", "data": "synthetic",
@@ -401,6 +412,8 @@ def run_gpu(args):
                               "achieved_tflops": per_gpu * FLOP_PER_CELL_UPDATE * 1e-12,
                               "achieved_gbs": per_gpu * BYTES_PER_CELL_UPDATE * 1e-9},
             "kernels": kernels,
+            "kernels_note": "per-kernel times from a SECOND pass of %d steps with a CUDA-event pair around every launch "
+                            "(%.3f ms/step in that pass); value / ms_per_step come from the first pass, timers off" % (Kk, ms_kpass / Kk),
             "state": {"t": d["t"], "max_div_b": d["max_div_b"], "c2p_mean_iters": d["c2p_mean_iters"],
                       "c2p_max_iters": d["c2p_max_iters"], "c2p_failures": d["c2p_failures"], "max_W": d["max_W"],
                       "min_rho": d["min_rho"], "min_p": d["min_p"]},
@@ -410,10 +423,37 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch and per CELL from the committed ncu --set full capture
-# (profiles/r1_ncu_full.md: 256^3, RK stage 2), keyed by kernel class; bench.py reports it times the cells of a launch.
-TRAFFIC_PER_CELL = {"k_prim": 206.0, "k_flux_x": 149.3, "k_flux_y": 177.3, "k_flux_z": 258.4, "k_uct": 164.2,
-                    "k_update": 95.8}
+def kernel_source_hash():
+    """sha256 over the CUDA sources the library is built from: ties an ncu capture to the kernels it measured."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2401_03008_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()
+
+
+def measured_traffic(kernel_class, cells, args):
+    """roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full
+    capture (profiles/r2_traffic.json, written by `python -m paper_2401_03008_b200.ncu_summary`), scaled from the
+    capture's cell count to this launch.  None, with the reason, when the capture is of other kernel sources, of
+    another scheme or absent: a stale number is worse than none."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if not os.path.exists(path):
+        return None, "no ncu capture committed (profiles/r2_traffic.json)"
+    with open(path) as f:
+        t = json.load(f)
+    if args.scheme != t.get("scheme", "uct-ho") or args.workload != "cpa":
+        return None, "the committed capture (profiles/r2_traffic.json) is of scheme %s on the cpa workload" % t.get("scheme")
+    if t.get("source_sha256") != kernel_source_hash():
+        return None, "profiles/r2_traffic.json was captured on other kernel sources (sha256 %s...)" % str(t.get("source_sha256"))[:12]
+    k = t.get("kernels", {}).get(kernel_class)
+    if not k:
+        return None, "kernel class %s is not in profiles/r2_traffic.json" % kernel_class
+    return k["dram_bytes_per_cell"] * cells, ("ncu dram__bytes_read.sum + dram__bytes_write.sum per cell of %s (%s, %d^3) x cells of "
+                                              "this launch; %s" % (k["kernel"], t.get("report"), t.get("n", 0), t.get("md")))
 
 
 def main():
@@ -425,6 +465,7 @@ def main():
     ap.add_argument("--n", type=int, default=256, help="box size n^3 (BASELINE.json configs[2]: 256)")
     ap.add_argument("--direction", default="diag", choices=["diag", "x"])
     ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--kernel-steps", type=int, default=10, help="steps of the second, per-kernel-timed pass")
     ap.add_argument("--e2e-lanes", type=int, default=3, help="handles/streams of the pipelined end-to-end measurement")
     ap.add_argument("--cpu-n", type=int, default=64)
     ap.add_argument("--cpu-steps", type=int, default=6)

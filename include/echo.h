@@ -41,7 +41,9 @@ typedef struct echo_ctx echo_ctx;
 
 /* Host only.  Periodic unit box of nx*ny*nz cells (each >= 1; a size-1 axis is legal and makes
  * the problem 2-D / 1-D through the periodic wrap), ideal-gas index gamma > 1 (eq.(6)),
- * Courant number cfl > 0 (dt = cfl * min_d h_d / a_max, S9).  Returns NULL on bad arguments. */
+ * Courant number cfl > 0 (dt = cfl * min_d h_d / a_max, S9).  Returns NULL on bad arguments, on
+ * nx*ny*nz >= 2^31 - 64 (32-bit cell indices) and on nz > 65535, ny > 262140 or (nz > 1 and ny > 65535)
+ * (grid-dimension limits of the launches). */
 echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl);
 
 /* Host only.  The paper's scheme switches, to be called before echo_set_primitives.
@@ -73,7 +75,9 @@ size_t echo_workspace_bytes(const echo_ctx *ctx);
 
 /* Binds a caller-owned device workspace (256-byte aligned, >= echo_workspace_bytes) and a CUDA
  * stream (cudaStream_t passed as void*; NULL = default stream).  The workspace must outlive the
- * handle.  Zero-fills the control block.  ECHO_ENOMEM if too small or misaligned. */
+ * handle.  Zero-fills the control block.  ECHO_ENOMEM if too small or misaligned, ECHO_EINVAL if it is
+ * not device memory.  The handle remembers the device the workspace lives on: every later call runs its
+ * kernels there (the stream must belong to that device) and restores the caller's current device. */
 int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
 
 /* Message of the last error on this handle (host string owned by the handle; "" if none). */
@@ -103,7 +107,8 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
 /* Advances nsteps full SSP-RK3 steps (O9; five points of a sub-step), or fewer if t
  * reaches t_end: the last dt is clipped to t_end - t on the device and later steps are no-ops
  * (pass +inf to disable).  The time step is formed on the device from the stage-1 characteristic
- * speeds of the same step (S9).  No host synchronisation. */
+ * speeds of the same step (S9).  No host synchronisation.  ECHO_EINVAL on a block
+ * handle with halos (echo_create_block): those are stepped stage by stage by their owner. */
 int echo_step(echo_ctx *ctx, int nsteps, double t_end);
 
 /* Host loop around echo_step: advances until t >= t_end (last dt clipped), max_steps steps were taken, or a
@@ -203,6 +208,14 @@ size_t echo_ctrl_offset(int what);
 /* First and second half of RK stage `stage` (1..3) of a block step; see above.  No synchronisation. */
 int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end);
 int echo_stage_finish(echo_ctx *ctx, int stage);
+
+/* Host only (needs the device of the bound workspace for the occupancy query).  The launch configuration in force
+ * for this handle, for tests that place samples across tile seams: out (HOST, 8 ints) = {cells per chunk of the
+ * x-, y-, z-sweep (an axis longer than 512 cells is cut into chunks; 1 for a one-cell axis), planes per z-chunk of
+ * the plane-marching INT+con2prim, UCT and curl+update kernels (0: that kernel is not used by this handle;
+ * negative: -(y-tiles per chunk) of the n_z = 1 variants marching along y), tile width, tile height of those
+ * kernels}. */
+int echo_get_tiling(echo_ctx *ctx, int *out);
 
 /* ---- measurement aids (used by bench.py; not part of the numerical path) -------------------- */
 

@@ -50,6 +50,7 @@ def lib():
         L.oracle_get_conserved.argtypes = [C.c_void_p] + [_dp] * 5
         L.oracle_rhs.argtypes = [C.c_void_p] + [C.POINTER(_dp)] * 4 + [_dp]
         L.oracle_con2prim.argtypes = [C.c_double, C.c_long] + [_dp] * 13 + [_ip]
+        L.oracle_con2prim_trace.argtypes = [C.c_double, C.c_long] + [_dp] * 13 + [_ip, _ip]
         L.oracle_prim2cons.argtypes = [C.c_double, C.c_long] + [_dp] * 13
         L.oracle_div_b.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_diagnostics.argtypes = [C.c_void_p, _dp]
@@ -177,6 +178,18 @@ def con2prim(gamma, D, Sx, Sy, Sz, U, Bx, By, Bz):
     rc = lib().oracle_con2prim(gamma, n, *[_p(a) for a in ins], *[_p(a) for a in outs],
                                iters.ctypes.data_as(_ip))
     return dict(rho=outs[0], vx=outs[1], vy=outs[2], vz=outs[3], p=outs[4], iters=iters, rc=rc)
+
+
+def con2prim_trace(gamma, D, Sx, Sy, Sz, U, Bx, By, Bz):
+    """con2prim + per-state count of safeguard activations (nsafe)."""
+    ins = [_c(a).ravel() for a in (D, Sx, Sy, Sz, U, Bx, By, Bz)]
+    n = ins[0].size
+    outs = [np.empty(n) for _ in range(5)]
+    iters = np.empty(n, dtype=np.int32)
+    nsafe = np.empty(n, dtype=np.int32)
+    rc = lib().oracle_con2prim_trace(gamma, n, *[_p(a) for a in ins], *[_p(a) for a in outs],
+                                     iters.ctypes.data_as(_ip), nsafe.ctypes.data_as(_ip))
+    return dict(rho=outs[0], vx=outs[1], vy=outs[2], vz=outs[3], p=outs[4], iters=iters, nsafe=nsafe, rc=rc)
 
 
 def prim2cons(gamma, rho, vx, vy, vz, p, Bx, By, Bz):

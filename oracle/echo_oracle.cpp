@@ -252,7 +252,8 @@ bool c2p_eval(double gam, double D, double S2, double B2, double T, double U, do
     return true;
 }
 
-int con2prim(double gam, const double u[5], const double B[3], double q[5]) {
+// nsafe (optional, instrumentation for the pins only): receives the number of times the safeguard replaced an iterate.
+int con2prim(double gam, const double u[5], const double B[3], double q[5], int *nsafe = nullptr) {
     const double tol = 1e-12;
     const int maxit = 30;
     const double D = u[0], *S = u + 1, U = u[4];
@@ -267,6 +268,7 @@ int con2prim(double gam, const double u[5], const double B[3], double q[5]) {
         if (!c2p_eval(gam, D, S2, B2, T, U, y, a)) {
             if (it == 0) break;  // the start itself is unphysical: fail
             ++it;                // safeguard: halve the step back towards the last valid iterate
+            if (nsafe) ++*nsafe;
             y = 0.5 * (y + ylast);
             if (!std::isfinite(y)) break;
             continue;
@@ -768,6 +770,24 @@ int oracle_con2prim(double gamma, long n, const double *D, const double *Sx, con
         const int it = con2prim(gamma, u, B, q);
         rho[c] = q[0]; vx[c] = q[1]; vy[c] = q[2]; vz[c] = q[3]; p[c] = q[4];
         if (iters) iters[c] = it;
+        if (it < 0) bad = 1;
+    }
+    return bad ? -5 : 0;
+}
+
+// the same, also reporting how often the safeguard of O2 replaced an iterate (nsafe[i]); same arithmetic
+int oracle_con2prim_trace(double gamma, long n, const double *D, const double *Sx, const double *Sy, const double *Sz,
+                          const double *U, const double *Bx, const double *By, const double *Bz, double *rho, double *vx,
+                          double *vy, double *vz, double *p, int *iters, int *nsafe) {
+    int bad = 0;
+    for (long c = 0; c < n; ++c) {
+        const double u[5] = {D[c], Sx[c], Sy[c], Sz[c], U[c]};
+        const double B[3] = {Bx[c], By[c], Bz[c]};
+        double q[5];
+        nsafe[c] = 0;
+        const int it = con2prim(gamma, u, B, q, &nsafe[c]);
+        rho[c] = q[0]; vx[c] = q[1]; vy[c] = q[2]; vz[c] = q[3]; p[c] = q[4];
+        iters[c] = it;
         if (it < 0) bad = 1;
     }
     return bad ? -5 : 0;

@@ -45,6 +45,7 @@ SIGNATURES = {
     "echo_ctrl_offset": (_sz, [_int]),
     "echo_stage_sweeps": (_int, [_vp, _int, _dbl]),
     "echo_stage_finish": (_int, [_vp, _int]),
+    "echo_get_tiling": (_int, [_vp, C.POINTER(_int)]),
     "echo_timing": (_int, [_vp, _int]),
     "echo_get_timing": (_int, [_vp, C.POINTER(_dbl), C.POINTER(_long)]),
     "echo_fp64_peak": (_int, [_int, C.POINTER(_dbl), _vp]),
@@ -90,8 +91,8 @@ def _dev(t, n=None):
     return t.data_ptr()
 
 
-def _stream():
-    return _torch().cuda.current_stream().cuda_stream
+def _stream(device=None):
+    return _torch().cuda.current_stream(device).cuda_stream
 
 
 class EchoError(RuntimeError):
@@ -125,7 +126,8 @@ class Echo:
             self._check(self.L.echo_set_order(self.h, int(rec), int(rk)))
         nbytes = self.L.echo_workspace_bytes(self.h)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned by the caller side
-        self._check(self.L.echo_bind(self.h, self.workspace.data_ptr(), nbytes, _stream()))
+        # the stream of the workspace's device: the library runs every kernel of this handle there (echo_bind)
+        self._check(self.L.echo_bind(self.h, self.workspace.data_ptr(), nbytes, _stream(self.device)))
 
     def __del__(self):
         if getattr(self, "h", None):
@@ -228,6 +230,13 @@ class Echo:
 
     def stage_finish(self, stage):
         self._check(self.L.echo_stage_finish(self.h, int(stage)))
+
+    def tiling(self):
+        """echo_get_tiling: the launch configuration in force (chunk lengths of the sweeps and marching kernels)."""
+        out = (_int * 8)()
+        self._check(self.L.echo_get_tiling(self.h, out))
+        names = ["cx_flux", "cy_flux", "cz_flux", "cz_prim", "cz_uct", "cz_bupd", "tile_x", "tile_y"]
+        return dict(zip(names, list(out)))
 
     # ---- measurement aids
     def timing(self, enable=True):

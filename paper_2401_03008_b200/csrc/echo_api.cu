@@ -26,6 +26,10 @@ struct echo_ctx {
     bool bound = false, has_state = false;
     int rk = 3;              // SSP-RK3 or SSP-RK2 (echo_set_order)
     bool block = false;      // echo_create_block: explicit spacing, halos refreshed by the caller between stages
+    bool gate_active = false;   // inside echo_step / echo_stage_*: con2prim failures count only while ctrl->active
+    int device = -1;         // device the bound workspace lives on (echo_bind); every launching call runs there
+    // launch configuration of the marching kernels (ensure_tiling; reported by echo_get_tiling)
+    struct Tiling { bool ready = false; int cz_prim = 0, cz_uct = 0, cz_bupd = 0, cy_uct_flat = 0, cy_bupd_flat = 0; } til;
     std::string err;
     // measurement aids (echo_timing / echo_get_timing)
     bool timing = false;
@@ -90,6 +94,24 @@ int resident_slots(K kernel, int threads) {
 }
 
 enum { KC_PRIM = 0, KC_FLUX = 1, KC_UCT = 4, KC_UPDATE = 5, KC_CTRL = 6, KC_OTHER = 7 };
+
+// chunk lengths of the plane-marching kernels for this handle's grid on this handle's device (once per handle)
+void ensure_tiling(echo_ctx *c) {
+    if (c->til.ready) return;
+    const Grid &g = c->g;
+    const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
+    c->til.cz_prim = pick_chunk_planes(tx * ty, g.n[2], resident_slots(k_prim_march<true>, UCT_NT), 2);
+    c->til.cz_uct = pick_chunk_planes(tx * ty, g.n[2], resident_slots(k_uct2<false>, UCT_NT), 3);
+    c->til.cz_bupd = pick_chunk_planes(tx * ty, g.n[2], resident_slots(k_bupd, UCT_NT), 2);
+    c->til.cy_uct_flat = pick_chunk_planes(tx, ty, resident_slots(k_uct2_flat<false>, UCT_NT), 3);
+    c->til.cy_bupd_flat = pick_chunk_planes(tx, ty, resident_slots(k_bupd_flat, UCT_NT), 2);
+    c->til.ready = true;
+}
+// chunk length of the flux sweep along D: one chunk per column unless the axis is long
+int flux_chunk_cells(const Grid &g, int D) {
+    const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
+    return (g.n[D] + nchunk - 1) / nchunk;
+}
 
 size_t next_event(echo_ctx *c) {
     if (c->ev_used == c->ev_pool.size()) {
@@ -158,8 +180,8 @@ int launch_flux_nt(echo_ctx *ctx, const Stage &st, int want_amax, const FluxUpd 
         return ECHO_OK;
     }
     // chunks along D: one chunk per column unless the axis is long (5 halo faces per chunk are recomputed)
-    const int nchunk = (g.n[D] + FLUX_CMAX - 1) / FLUX_CMAX;
-    const int C = (g.n[D] + nchunk - 1) / nchunk;
+    const int C = flux_chunk_cells(g, D);
+    const int nchunk = (g.n[D] + C - 1) / C;
     dim3 grid((g.n[TD] + T - 1) / T, nchunk, g.n[OD]);
     if (!g.uct) {   // UCT = NO: 8 flux components, rings of 49 KB in dynamic shared memory
         constexpr int R = NT / T, RL = 3 * R, SB = RL + 4;   // as in k_flux
@@ -209,25 +231,25 @@ int launch_sweeps(echo_ctx *ctx, const Stage &st, int want_amax, const StagePlan
     PrimUpd pu;
     for (int v = 0; v < 8; ++v) pu.uout[v] = ctx->field[F_U1 + v];
     for (int d = 0; d < 3; ++d) pu.bin[d] = ctx->field[F_BF + d];
+    const int *gate = ctx->gate_active ? &ctx->ctrl->active : &ctx->ctrl->one;
     if (!g.uct) {
         if (pl && pl->prim_upd)
-            KL(KC_PRIM, "k_prim_cc", k_prim<false, true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+            KL(KC_PRIM, "k_prim_cc", k_prim<false, true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, gate));
         else
-            KL(KC_PRIM, "k_prim_cc", k_prim<false, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+            KL(KC_PRIM, "k_prim_cc", k_prim<false, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, gate));
     } else if (g.n[2] < 8) {   // a thin grid (2.5-D runs): nothing to march along, the thread-per-cell kernel is faster
         if (pl && pl->prim_upd)
-            KL(KC_PRIM, "k_prim", k_prim<false, true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+            KL(KC_PRIM, "k_prim", k_prim<false, true><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, gate));
         else
-            KL(KC_PRIM, "k_prim", k_prim<false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu));
+            KL(KC_PRIM, "k_prim", k_prim<false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, gate));
     } else {   // plane-marching INT + con2prim (k_prim_march), tiles and z-chunks as for k_bupd
-        const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
-        static const int slots = resident_slots(k_prim_march<true>, UCT_NT);
-        const int CZ = pick_chunk_planes(tiles, g.n[2], slots, 2);
+        ensure_tiling(ctx);
+        const int CZ = ctx->til.cz_prim;
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
         if (pl && pl->prim_upd)
-            KL(KC_PRIM, "k_prim_march", k_prim_march<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, CZ));
+            KL(KC_PRIM, "k_prim_march", k_prim_march<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, CZ, gate));
         else
-            KL(KC_PRIM, "k_prim_march", k_prim_march<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, CZ));
+            KL(KC_PRIM, "k_prim_march", k_prim_march<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, pu, CZ, gate));
     }
     FluxUpd fu;
     for (int v = 0; v < 8; ++v) {
@@ -256,16 +278,15 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
         // against 1.21 ms for the single kernel at 256^3, so the single kernel stays)
         if (g.n[2] == 1) {   // 2.5-D: the same kernel marching along y (k_uct2_flat)
             const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
-            static const int fslots = resident_slots(k_uct2_flat<false>, UCT_NT);
-            const int CY = pick_chunk_planes(tx, ty, fslots, 3);
+            ensure_tiling(ctx);
+            const int CY = ctx->til.cy_uct_flat;
             dim3 grid(tx, (ty + CY - 1) / CY, 1);
             if (g.rec == 2) KL(KC_UCT, "k_uct2_flat", k_uct2_flat<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CY));
             else KL(KC_UCT, "k_uct2_flat", k_uct2_flat<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CY));
             return ECHO_OK;
         }
-        const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
-        static const int slots = resident_slots(k_uct2<false>, UCT_NT);
-        const int CZ = pick_chunk_planes(tiles, g.n[2], slots, 3);
+        ensure_tiling(ctx);
+        const int CZ = ctx->til.cz_uct;
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
         if (g.rec == 2) KL(KC_UCT, "k_uct2", k_uct2<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
         else KL(KC_UCT, "k_uct2", k_uct2<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
@@ -300,19 +321,36 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
                                                                               st.R[2], st.R[3], st.R[4], up, ctx->ctrl, 1));
     } else if (g.n[2] == 1) {   // 2.5-D: curl + update marching along y (k_bupd_flat)
         const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
-        static const int fslots = resident_slots(k_bupd_flat, UCT_NT);
-        const int CY = pick_chunk_planes(tx, ty, fslots, 2);
+        ensure_tiling(ctx);
+        const int CY = ctx->til.cy_bupd_flat;
         dim3 grid(tx, (ty + CY - 1) / CY, 1);
         KL(KC_UPDATE, "k_bupd_flat", k_bupd_flat<<<grid, UCT_NT, 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], up, ctx->ctrl, CY));
     } else {   // staggered B only: plane-marching curl + update
-        const int tiles = ((g.n[0] + UCT_TX - 1) / UCT_TX) * ((g.n[1] + UCT_TY - 1) / UCT_TY);
-        static const int slots = resident_slots(k_bupd, UCT_NT);
-        const int CZ = pick_chunk_planes(tiles, g.n[2], slots, 2);
+        ensure_tiling(ctx);
+        const int CZ = ctx->til.cz_bupd;
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
         KL(KC_UPDATE, "k_bupd", k_bupd<<<grid, UCT_NT, 0, ctx->stream>>>(g, st.E[0], st.E[1], st.E[2], up, ctx->ctrl, CZ));
     }
     return ECHO_OK;
 }
+
+// Every launching call runs on the device of the bound workspace, whatever the calling thread's current device is,
+// and leaves the caller's current device as it found it.
+struct DevGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DevGuard(const echo_ctx *c) {
+        if (c && c->device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+struct GateScope {   // echo_step / echo_stage_sweeps: see echo_ctx::gate_active
+    echo_ctx *c;
+    explicit GateScope(echo_ctx *ctx) : c(ctx) { c->gate_active = true; }
+    ~GateScope() { c->gate_active = false; }
+};
 
 int check_ready(echo_ctx *ctx, bool need_state) {
     if (!ctx) return ECHO_EINVAL;
@@ -328,7 +366,8 @@ extern "C" {
 echo_ctx *echo_create(int nx, int ny, int nz, double gamma, double cfl) {
     if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || !(cfl > 0.0) || !std::isfinite(gamma) || !std::isfinite(cfl))
         return nullptr;
-    if ((long long)nx * ny * nz >= (1LL << 31) - 64 || nz > 65535 || ny > 4 * 65535) return nullptr;   // 32-bit cell indices
+    // 32-bit cell indices; grid-dimension limits of the launches (the z-sweep puts y on gridDim.z when nz > 1)
+    if ((long long)nx * ny * nz >= (1LL << 31) - 64 || nz > 65535 || ny > 4 * 65535 || (nz > 1 && ny > 65535)) return nullptr;
     echo_ctx *c = new (std::nothrow) echo_ctx();
     if (!c) return nullptr;
     Grid &g = c->g;
@@ -360,6 +399,14 @@ int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     if (!ctx) return ECHO_EINVAL;
     if (!dev_workspace || bytes < echo_workspace_bytes(ctx) || ((size_t)dev_workspace & 255))
         return fail(ctx, ECHO_ENOMEM, "workspace missing, misaligned or smaller than echo_workspace_bytes");
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, dev_workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return fail(ctx, ECHO_EINVAL, "the workspace is not device memory");
+    }
+    ctx->device = attr.device;
+    DevGuard dev_guard_(ctx);
+    ctx->til.ready = false;
     ctx->ws = static_cast<char *>(dev_workspace);
     ctx->ws_bytes = bytes;
     ctx->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -381,6 +428,7 @@ int echo_set_primitives(echo_ctx *ctx, const double *rho, const double *vx, cons
                         const double *p, const double *bxf, const double *byf, const double *bzf) {
     int rc = check_ready(ctx, false);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (!rho || !vx || !vy || !vz || !p || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
     const Grid &g = ctx->g;
     const double *bf[3] = {bxf, byf, bzf};
@@ -391,6 +439,8 @@ int echo_set_primitives(echo_ctx *ctx, const double *rho, const double *vx, cons
                                                            ctx->field[F_BF + 2], ctx->field[F_U], ctx->field[F_U + 1],
                                                            ctx->field[F_U + 2], ctx->field[F_U + 3], ctx->field[F_U + 4],
                                                            ctx->gg));
+    // the stage buffers are read (never trusted) by the passes of a step enqueued past t_end: give them defined contents
+    CU(cudaMemsetAsync(ctx->field[F_U1], 0, sizeof(double) * (size_t)ctx->npad * 8, ctx->stream));
     Ctrl h;
     std::memset(&h, 0, sizeof(h));
     h.one = 1;
@@ -404,6 +454,7 @@ int echo_set_primitives_host(echo_ctx *ctx, const double *rho, const double *vx,
                              const double *p, const double *bxf, const double *byf, const double *bzf) {
     int rc = check_ready(ctx, false);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (!rho || !vx || !vy || !vz || !p || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
     const size_t nb = sizeof(double) * ctx->g.N;
     const double *src[8] = {rho, vx, vy, vz, p, bxf, byf, bzf};
@@ -418,6 +469,7 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
                               double b0y, double b0z, double *bxf, double *byf, double *bzf) {
     int rc = check_ready(ctx, false);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (!ax || !ay || !az || !bxf || !byf || !bzf) return fail(ctx, ECHO_EINVAL, "null array");
     const Grid &g = ctx->g;
     KL(KC_OTHER, "k_curl", k_curl<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, ax, ay, az, bxf, byf, bzf, -1.0, b0x, b0y, b0z));
@@ -427,7 +479,11 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
 int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
+    if (ctx->block && (ctx->g.lo[0] > 0 || ctx->g.lo[1] > 0 || ctx->g.lo[2] > 0))
+        return fail(ctx, ECHO_EINVAL, "a block with halos is stepped stage by stage (echo_stage_sweeps / echo_stage_finish) by its owner");
+    GateScope gate_scope_(ctx);
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     const bool rk2 = ctx->rk == 2;   // SSP-RK2 (O3b): stage 1 as below, then U^{n+1} = 1/2 U^n + 1/2 (U1 + dt L(U1))
     if (!ctx->g.uct) {
@@ -476,6 +532,7 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
 int echo_run_until(echo_ctx *ctx, double t_end, long max_steps, long *steps_taken_host) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (std::isnan(t_end) || max_steps < 0) return fail(ctx, ECHO_EINVAL, "t_end is NaN or max_steps < 0");
     if (ctx->block) return fail(ctx, ECHO_EINVAL, "block handles are stepped stage by stage by their owner");
     Ctrl h;
@@ -506,14 +563,15 @@ int echo_get_primitives(echo_ctx *ctx, double *rho, double *vx, double *vy, doub
                         double *byc, double *bzc, double *bxf, double *byf, double *bzf) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (!rho || !vx || !vy || !vz || !p || !bxc || !byc || !bzc) return fail(ctx, ECHO_EINVAL, "null array");
     const Grid &g = ctx->g;
     Stage st = make_stage(ctx, 0);
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 5; ++v) st.P[v] = out[v];
     for (int d = 0; d < 3; ++d) st.Bc[d] = out[5 + d];
-    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
-    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd(), &ctx->ctrl->one));
+    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd(), &ctx->ctrl->one));
     double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d)
         if (bf[d]) CU(cudaMemcpyAsync(bf[d], ctx->field[F_BF + d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -525,12 +583,13 @@ static int get_primitives_host_impl(echo_ctx *ctx, double *rho, double *vx, doub
                                     bool sync) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (!rho || !vx || !vy || !vz || !p || !bxc || !byc || !bzc) return fail(ctx, ECHO_EINVAL, "null array");
     const Grid &g = ctx->g;
     const size_t nb = sizeof(double) * g.N;
     Stage st = make_stage(ctx, 0);
-    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
-    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd(), &ctx->ctrl->one));
+    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd(), &ctx->ctrl->one));
     double *out[8] = {rho, vx, vy, vz, p, bxc, byc, bzc};
     for (int v = 0; v < 8; ++v) CU(cudaMemcpyAsync(out[v], ctx->field[F_P + v], nb, cudaMemcpyDeviceToHost, ctx->stream));
     double *bf[3] = {bxf, byf, bzf};
@@ -553,6 +612,7 @@ int echo_get_primitives_host_async(echo_ctx *ctx, double *rho, double *vx, doubl
 int echo_synchronize(echo_ctx *ctx) {
     int rc = check_ready(ctx, false);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     CU(cudaStreamSynchronize(ctx->stream));
     return ECHO_OK;
 }
@@ -560,6 +620,7 @@ int echo_synchronize(echo_ctx *ctx) {
 int echo_get_conserved(echo_ctx *ctx, double *D, double *Sx, double *Sy, double *Sz, double *U) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     double *out[5] = {D, Sx, Sy, Sz, U};
     for (int v = 0; v < 5; ++v) {
         if (!out[v]) return fail(ctx, ECHO_EINVAL, "null array");
@@ -571,6 +632,7 @@ int echo_get_conserved(echo_ctx *ctx, double *D, double *Sx, double *Sy, double 
 int echo_rhs(echo_ctx *ctx, double *const *rhsU, double *const *rhsB, double *const *E, double *amax_host) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     const Grid &g = ctx->g;
     const size_t nb = sizeof(double) * g.N;
     const Stage st = make_stage(ctx, 0);
@@ -624,6 +686,7 @@ int echo_prim2cons(double gamma, long n, const double *rho, const double *vx, co
 int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     const Grid &g = ctx->g;
     double *slot = ctx->part + 15 * NPART;   // spare partial row: one double for the max
     CU(cudaMemsetAsync(slot, 0, sizeof(double), ctx->stream));
@@ -639,6 +702,7 @@ int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host) {
 int echo_diagnostics(echo_ctx *ctx, double *out) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (!out) return fail(ctx, ECHO_EINVAL, "null output");
     const Grid &g = ctx->g;
     for (int m = 0; m < ECHO_NDIAG; ++m) out[m] = 0.0;
@@ -648,8 +712,8 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
                                            f + 7 * np, ctx->part));
     Stage st = make_stage(ctx, 0);
     KL(KC_CTRL, "k_c2p_stats_reset", k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
-    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
-    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd()));
+    if (g.uct) KL(KC_PRIM, "k_prim", k_prim<true, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd(), &ctx->ctrl->one));
+    else KL(KC_PRIM, "k_prim_cc", k_prim<true, false, false><<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, st, ctx->gamma, ctx->ctrl, PrimUpd(), &ctx->ctrl->one));
     KL(KC_OTHER, "k_extrema", k_extrema<<<NPART, 256, 0, ctx->stream>>>(g.N, st.P[0], st.P[1], st.P[2], st.P[3], st.P[4], ctx->part));
     double dmax = 0.0;
     if ((rc = echo_div_b(ctx, nullptr, &dmax))) return rc;   // synchronises
@@ -741,9 +805,11 @@ size_t echo_ctrl_offset(int what) {
 int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
     if (!ctx->g.uct || ctx->rk != 3) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES and SSP-RK3 only");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    GateScope gate_scope_(ctx);
     if (stage == 1) {
         KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
         return launch_sweeps(ctx, s0, 2);
@@ -756,6 +822,7 @@ int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
 int echo_stage_finish(echo_ctx *ctx, int stage) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
     if (!ctx->g.uct || ctx->rk != 3) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES and SSP-RK3 only");
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
@@ -772,9 +839,27 @@ int echo_stage_finish(echo_ctx *ctx, int stage) {
     return ECHO_OK;
 }
 
+int echo_get_tiling(echo_ctx *ctx, int *out) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    DevGuard dev_guard_(ctx);
+    if (!out) return fail(ctx, ECHO_EINVAL, "null output");
+    ensure_tiling(ctx);
+    const Grid &g = ctx->g;
+    for (int d = 0; d < 3; ++d) out[d] = g.n[d] == 1 ? 1 : flux_chunk_cells(g, d);
+    const bool march = g.n[2] >= 8;        // thin grids keep the thread-per-cell k_prim
+    out[3] = (g.uct && march) ? ctx->til.cz_prim : 0;
+    out[4] = !g.uct ? 0 : (g.n[2] == 1 ? -ctx->til.cy_uct_flat : ctx->til.cz_uct);
+    out[5] = !g.uct ? 0 : (g.n[2] == 1 ? -ctx->til.cy_bupd_flat : ctx->til.cz_bupd);
+    out[6] = UCT_TX;
+    out[7] = UCT_TY;
+    return ECHO_OK;
+}
+
 int echo_timing(echo_ctx *ctx, int enable) {
     int rc = check_ready(ctx, false);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     CU(cudaStreamSynchronize(ctx->stream));
     ctx->timing = enable != 0;
     ctx->spans.clear();
@@ -786,6 +871,7 @@ int echo_timing(echo_ctx *ctx, int enable) {
 int echo_get_timing(echo_ctx *ctx, double *ms_total, long *launches) {
     int rc = check_ready(ctx, false);
     if (rc) return rc;
+    DevGuard dev_guard_(ctx);
     CU(cudaStreamSynchronize(ctx->stream));
     if (ms_total) {
         for (int c = 0; c < ECHO_NKCLASS; ++c) ms_total[c] = 0.0;

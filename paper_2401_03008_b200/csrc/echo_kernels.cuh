@@ -62,10 +62,11 @@ __global__ void k_c2p_stats_reset(Ctrl *c) {
 // spare memory bandwidth, so the update costs no pass of its own and U1 is never re-read.
 // UCT = false: B is a cell-centred evolved field (st.Bf holds it); no INT, and the deferred update covers B too
 // (bin = B^n, rhs of B in st.E, result to uout[5..7]).
+// gate: device flag that must be non-zero for a con2prim failure to be counted (ctrl->active or ctrl->one).
 struct PrimUpd { double *uout[8]; const double *bin[3]; };
 
 template <bool STATS, bool UPD, bool UCT = true>
-__global__ void __launch_bounds__(256, 5) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu) {
+__global__ void __launch_bounds__(256, 5) k_prim(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu, const int *gate) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
@@ -106,7 +107,9 @@ __global__ void __launch_bounds__(256, 5) k_prim(Grid g, Stage st, double gam, C
         for (int v = 0; v < 5; ++v) st.P[v][c] = q[v];
 #pragma unroll
         for (int d = 0; d < 3; ++d) st.Bc[d][c] = B[d];
-        if (it < 0 && i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2])
+        // failures are counted in the interior of a block only, and (gate = &ctrl->active inside echo_step) not by
+        // the passes of a step enqueued past t_end, which run on stale stage buffers; the load sits in the rare branch
+        if (it < 0 && i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2] && *gate)
             atomicAdd(&ctrl->c2p_fail_total, 1ull);
     }
     if (STATS) {

@@ -548,7 +548,8 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd_flat(Grid g, const double *E0, 
 namespace echo {
 
 template <bool UPD>
-__global__ void __launch_bounds__(UCT_NT) k_prim_march(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu, int CZ) {
+__global__ void __launch_bounds__(UCT_NT) k_prim_march(Grid g, Stage st, double gam, Ctrl *ctrl, PrimUpd pu, int CZ,
+                                                       const int *gate) {
     __shared__ double sBX[2][BU_XE];       // B_x, x offsets -3 .. TX+1
     __shared__ double sBY[2][BU_YE];       // B_y, y offsets -3 .. TY+1
     const int tid = threadIdx.x;
@@ -631,7 +632,7 @@ __global__ void __launch_bounds__(UCT_NT) k_prim_march(Grid g, Stage st, double 
             for (int v = 0; v < 5; ++v) st.P[v][o] = q[v];
 #pragma unroll
             for (int d = 0; d < 3; ++d) st.Bc[d][o] = B[d];
-            if (it < 0 && inxy && k >= g.lo[2] && k < g.hi[2]) atomicAdd(&ctrl->c2p_fail_total, 1ull);
+            if (it < 0 && inxy && k >= g.lo[2] && k < g.hi[2] && *gate) atomicAdd(&ctrl->c2p_fail_total, 1ull);
         }
 #pragma unroll
         for (int m = 0; m < 5; ++m) wz[m] = wz[m + 1];

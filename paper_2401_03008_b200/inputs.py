@@ -228,11 +228,13 @@ def turbulence_2d(nx, ny=None, seed=2401, eta_mean=0.25, gamma=4.0 / 3.0):
 
 
 # --------------------------------------------------------------------------------------
-def random_states(n, seed=12345, gamma=4.0 / 3.0, wmax=10.0, sigma_max=10.0):
+def random_states(n, seed=12345, gamma=4.0 / 3.0, wmax=10.0, sigma_max=10.0, wmin=1.0, log_p_over_rho=(-2.0, 2.0)):
     """P6 sample: random primitive states up to Lorentz factor wmax and magnetisation sigma_max.
 
     rho ~ logU[1e-2,1e2], p/rho ~ logU[1e-2,1e2], u = W v uniform in [0, sqrt(wmax^2-1)] with an
     isotropic direction, sigma = b^2/(rho h) ~ logU[1e-3, sigma_max] with isotropic B direction.
+    wmin > 1 and a colder log10(p/rho) range give the ultra-relativistic cold states (W of 20-40, p/rho of
+    1e-6..1e-2) on which the Newton iteration of con2prim leaves its domain and needs its safeguard (O2).
     """
     rng = np.random.default_rng(seed)
 
@@ -243,8 +245,8 @@ def random_states(n, seed=12345, gamma=4.0 / 3.0, wmax=10.0, sigma_max=10.0):
         return np.stack([st * np.cos(ph), st * np.sin(ph), mu])
 
     rho = 10.0 ** rng.uniform(-2.0, 2.0, n)
-    p = rho * 10.0 ** rng.uniform(-2.0, 2.0, n)
-    u = rng.uniform(0.0, math.sqrt(wmax * wmax - 1.0), n)
+    p = rho * 10.0 ** rng.uniform(log_p_over_rho[0], log_p_over_rho[1], n)
+    u = rng.uniform(math.sqrt(wmin * wmin - 1.0), math.sqrt(wmax * wmax - 1.0), n)
     W = np.sqrt(1.0 + u * u)
     v = iso(n) * (u / W)
     sigma = 10.0 ** rng.uniform(-3.0, math.log10(sigma_max), n)

@@ -46,6 +46,10 @@ def test_host_only_calls(libpath):
     assert not L.echo_create(0, 1, 1, 4.0 / 3.0, 0.3)
     assert not L.echo_create(8, 8, 8, 0.9, 0.3)
     assert not L.echo_create(8, 8, 8, 4.0 / 3.0, -1.0)
+    assert not L.echo_create(2, 70000, 2, 4.0 / 3.0, 0.3)                # the z-sweep puts y on gridDim.z
+    h2 = L.echo_create(2, 70000, 1, 4.0 / 3.0, 0.3)                      # a flat grid does not
+    assert h2
+    L.echo_destroy(h2)
     h = L.echo_create(8, 6, 4, 4.0 / 3.0, 0.3)
     assert h
     n = 8 * 6 * 4

@@ -16,12 +16,45 @@ SETK = "rho vx vy vz p bxf byf bzf".split()
 PRIMS = "rho vx vy vz p bx by bz".split()
 
 
+def subbox_check(ob, w, q, n, dt, centres, m=64, inner=8, tight=1e-12):
+    """The oracle advances an m^3 periodic sub-box cut out of the initial data `w` (n^3) around each centre
+    (x, y, z) by one step of the same dt; the inner `inner`^3 cells must agree with the full-size CUDA result q."""
+    lo = (m - inner) // 2
+    sl = slice(lo, lo + inner)
+    for centre in centres:
+        ix = [(np.arange(m) + c - m // 2) % n for c in centre]
+        sub = {k: np.ascontiguousarray(w[k][np.ix_(ix[2], ix[1], ix[0])]) for k in SETK}
+        o = ob.Oracle(m, m, m, G, 1e3)                                   # cfl so large that dt = t_end
+        o.set_primitives(*[sub[k] for k in SETK])
+        assert o.step(1, dt * n / m) == 1
+        assert o.diagnostics()["dt_last"] == dt * n / m
+        qo = o.get_primitives()
+        for k in PRIMS + ["bxf", "byf", "bzf"]:
+            ref = qo[k][sl, sl, sl]
+            got = q[k][np.ix_(ix[2][sl], ix[1][sl], ix[0][sl])]
+            err = np.abs(got - ref).max() / np.abs(qo[k]).max()                 # S16 norm
+            assert err <= 1e-10, (centre, k, err)
+            assert err <= tight, ("above round-off level", centre, k, err)
+
+
+def seam_planes(e):
+    """First plane of every z-chunk but the first of the plane-marching kernels (echo_get_tiling): where their
+    register / shared-memory windows restart."""
+    t = e.tiling()
+    out = set()
+    for key in ("cz_prim", "cz_uct", "cz_bupd"):
+        cz = t[key]
+        if 0 < cz < e.n[2]:
+            out.update(range(cz, e.n[2], cz))
+    return sorted(out), t
+
+
 def test_256_sampled_parity_and_invariants():
     import torch
     from paper_2401_03008_b200 import binding as eb
     from oracle import binding as ob
 
-    n, m, inner = 256, 64, 8
+    n = 256
     w = inputs.cpa_wave(n, n, n)
     e = eb.Echo(n, n, n, G, 0.3)
     e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
@@ -33,23 +66,12 @@ def test_256_sampled_parity_and_invariants():
     assert dt == pytest.approx(0.3 / n / d1["amax"], rel=1e-14)          # S9, on the device
     q = {k: v.cpu().numpy() for k, v in e.get_primitives().items()}
 
-    # ---- sampled outputs recomputed by the oracle
-    lo = (m - inner) // 2
-    for centre in [(0, 0, 0), (100, 37, 201), (255, 128, 5)]:            # (x, y, z) incl. the periodic seams
-        ix = [(np.arange(m) + c - m // 2) % n for c in centre]
-        sub = {k: np.ascontiguousarray(w[k][np.ix_(ix[2], ix[1], ix[0])]) for k in SETK}
-        o = ob.Oracle(m, m, m, G, 1e3)                                   # cfl so large that dt = t_end
-        o.set_primitives(*[sub[k] for k in SETK])
-        assert o.step(1, dt * n / m) == 1
-        assert o.diagnostics()["dt_last"] == dt * n / m
-        qo = o.get_primitives()
-        sl = slice(lo, lo + inner)
-        for k in PRIMS + ["bxf", "byf", "bzf"]:
-            ref = qo[k][sl, sl, sl]
-            got = q[k][np.ix_(ix[2][sl], ix[1][sl], ix[0][sl])]
-            err = np.abs(got - ref).max() / np.abs(qo[k]).max()
-            assert err <= 1e-10, (centre, k, err)
-            assert err <= 1e-12, ("above round-off level", centre, k, err)
+    # ---- sampled outputs recomputed by the oracle: the periodic seams, an interior point, and a box whose inner
+    # cells straddle a z-chunk seam of the plane-marching kernels (computed from the launch configuration in force)
+    seams, til = seam_planes(e)
+    assert seams, til                                                   # 256 planes are cut into several chunks
+    zs = seams[len(seams) // 2]
+    subbox_check(ob, w, q, n, dt, [(0, 0, 0), (100, 37, 201), (255, 128, 5), (77, 130, zs), (8, 251, seams[-1])])
 
     # ---- properties at full size
     assert d1["max_div_b"] * (1.0 / n) <= 1e-12 * 2.0                    # P5 (|B| <= 2)
@@ -63,3 +85,65 @@ def test_256_sampled_parity_and_invariants():
     ex = inputs.cpa_wave(n, n, n, t=d1["t"])
     for k in PRIMS:
         assert np.abs(q[k] - ex[k]).max() <= 1e-8, k
+
+
+def test_384_turbulence_sampled_parity():
+    """BASELINE.json configs[4] at its full size (384^3 Alfvenic turbulence, the launch configuration bench.py
+    --workload turb3d times): one step, sampled sub-boxes recomputed by the oracle (the trick is field-agnostic:
+    the periodic images of the cut only reach 24 cells in one step), div B and conservation at full size."""
+    import torch
+    from paper_2401_03008_b200 import binding as eb
+    from oracle import binding as ob
+
+    n = 384
+    w = inputs.turbulence(n)
+    e = eb.Echo(n, n, n, G, 0.3)
+    faces = e.faces_from_potential(*[torch.as_tensor(w[k], device="cuda") for k in ("ax", "ay", "az")], w["b0"])
+    for k, f in zip(("bxf", "byf", "bzf"), faces):
+        w[k] = f.cpu().numpy()
+    del faces
+    for k in ("ax", "ay", "az"):
+        del w[k]
+    e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
+    d0 = e.diagnostics()
+    e.step(1)
+    d1 = e.diagnostics()
+    assert d1["rc"] == 0 and d1["steps"] == 1 and d1["c2p_failures"] == 0
+    dt = d1["dt_last"]
+    assert dt == pytest.approx(0.3 / n / d1["amax"], rel=1e-14)
+    q = {k: v.cpu().numpy() for k, v in e.get_primitives().items()}
+    seams, til = seam_planes(e)
+    assert seams, til
+    subbox_check(ob, w, q, n, dt, [(0, 0, 0), (383, 200, 17), (150, 301, seams[0]), (9, 64, seams[-1])], tight=1e-11)
+    assert d1["max_div_b"] <= 1e-12 * w["B0"] * n * 50                   # P5 on a multi-mode field
+    for k in ("sum_D", "sum_Sx", "sum_Sy", "sum_Sz", "sum_U", "sum_Bx", "sum_By", "sum_Bz"):
+        assert abs(d1[k] - d0[k]) <= 1e-12 * max(abs(d0[k]), 1.0), k    # P4
+
+
+def test_512_x_aligned_sampled_parity():
+    """BASELINE.json configs[3], the x-aligned wave at 512^3 (47 GB workspace, the launch configuration bench.py
+    --n 512 --direction x times): one step, sampled sub-boxes recomputed by the oracle, the y/z independence of
+    the x-aligned wave bit for bit, div B and conservation."""
+    import torch
+    from paper_2401_03008_b200 import binding as eb
+    from oracle import binding as ob
+
+    n = 512
+    w = inputs.cpa_wave(n, n, n, direction="x")
+    e = eb.Echo(n, n, n, G, 0.3)
+    e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
+    d0 = e.diagnostics()
+    e.step(1)
+    d1 = e.diagnostics()
+    assert d1["rc"] == 0 and d1["steps"] == 1
+    dt = d1["dt_last"]
+    assert dt == pytest.approx(0.3 / n / d1["amax"], rel=1e-14)
+    q = {k: v.cpu().numpy() for k, v in e.get_primitives().items()}
+    seams, til = seam_planes(e)
+    subbox_check(ob, w, q, n, dt, [(0, 0, 0), (511, 300, seams[0] if seams else 100)])
+    for k in PRIMS:                                                      # P7(i): no dependence on y, z, bitwise
+        a = q[k]
+        assert np.array_equal(a, np.broadcast_to(a[:1, :1, :], a.shape)), k
+    assert d1["max_div_b"] * (1.0 / n) <= 1e-12 * 2.0
+    for k in ("sum_D", "sum_Sx", "sum_Sy", "sum_Sz", "sum_U", "sum_Bx", "sum_By", "sum_Bz"):
+        assert abs(d1[k] - d0[k]) <= 1e-12 * max(abs(d0[k]), 1.0), k

@@ -496,3 +496,64 @@ def test_two_runs_are_bit_identical(torch, eb, ob):
     assert outs[0][1] == outs[1][1]
     for a, b in zip(outs[0][0], outs[1][0]):
         assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("shape,roll", [((1100, 6, 2), (0, 0, 700)), ((6, 1100, 1), (0, 433, 0)), ((4, 6, 1100), (541, 0, 0)),
+                                        ((6, 1030, 3), (0, 7, 0))])
+def test_long_axis_multi_chunk_sweeps(torch, eb, ob, shape, roll):
+    """k_flux with MORE THAN ONE chunk along the sweep axis (an axis longer than FLUX_CMAX = 512 cells is cut
+    into chunks whose first five faces are recomputed by the neighbouring chunk, csrc/echo_api.cu launch_flux_nt)
+    - the path every column of the 4096^2 run of row f3 goes through.  Long thin boxes of the multi-mode
+    config-5 field: L(U) and 6 steps against the oracle, and bitwise translation covariance under a roll (z, y, x)
+    that moves the data across the chunk seams (1100 cells -> 3 chunks of 367, seams at 367 and 734)."""
+    w = turb_inputs(torch, eb, ob, None, shape=shape)
+    e, o = make_pair(torch, eb, ob, w, shape)
+    rg, ro = e.rhs(), o.rhs()
+    assert rg["amax"] == pytest.approx(ro["amax"], rel=1e-14)
+    for name in ("rhsU", "rhsB", "E"):
+        for c in range(len(ro[name])):
+            assert absinf(rg[name][c].cpu().numpy(), ro[name][c]) <= 1e-11 * max(1.0, np.abs(ro[name][c]).max()), (name, c)
+    e.step(6)
+    assert o.step(6) == 6
+    compare_prims(e, o, tight=1e-11)
+    dg, do = e.diagnostics(), o.diagnostics()
+    assert dg["t"] == pytest.approx(do["t"], rel=1e-13) and dg["c2p_failures"] == 0
+    for k in ("sum_D", "sum_Sx", "sum_Sy", "sum_Sz", "sum_U", "sum_Bx", "sum_By", "sum_Bz"):
+        assert dg[k] == pytest.approx(do[k], rel=1e-12, abs=1e-13), k            # P4 across the chunk seams
+    assert dg["max_div_b"] <= 1e-12 * w["B0"] * max(shape) * 50
+    rl = lambda a: np.roll(a, roll, axis=(0, 1, 2))
+    e1 = eb.Echo(*shape, G, 0.3)
+    e1.set_primitives(*[dev(torch, rl(w[k])) for k in SETK])
+    e1.step(6)
+    q0, q1 = e.get_primitives(), e1.get_primitives()
+    for k in q0:
+        assert np.array_equal(rl(q0[k].cpu().numpy()), q1[k].cpu().numpy()), k
+
+
+def test_steps_past_t_end_leave_state_and_failure_count_alone(torch, eb, ob):
+    """echo_step(n, t_end <= t) on a FRESH handle: the passes of such steps still run (on zeroed stage buffers), must
+    leave the state bit for bit unchanged and must not count their con2prim failures; echo_step refuses block handles
+    with halos; echo_get_tiling reports the launch configuration."""
+    shape = (24, 16, 12)
+    w = turb_inputs(torch, eb, ob, None, shape=shape)
+    e = eb.Echo(*shape, G, 0.3)
+    e.set_primitives(*[dev(torch, w[k]) for k in SETK])
+    q0 = {**e.get_primitives(), **e.get_conserved()}
+    e.step(3, 0.0)
+    d = e.diagnostics()
+    assert d["rc"] == 0 and d["c2p_failures"] == 0 and d["steps"] == 0 and d["t"] == 0.0
+    q1 = {**e.get_primitives(), **e.get_conserved()}
+    for k in q0:
+        assert torch.equal(q0[k], q1[k]), k
+    e.step(2)                                             # and the handle still steps normally afterwards
+    o = ob.Oracle(*shape, G, 0.3)
+    o.set_primitives(*[w[k] for k in SETK])
+    o.step(2)
+    compare_prims(e, o, tight=1e-11)
+    blk = eb.Echo(24, 8, 8, G, 0.3, block=(16, 8, 8, 8, 0, 0))
+    z = [torch.ones(8, 8, 24, dtype=torch.float64, device="cuda") * c for c in (1, 0, 0, 0, 1, 1, 0, 0)]
+    blk.set_primitives(*z)
+    assert blk.L.echo_step(blk.h, 1, math.inf) == eb.ECHO_EINVAL
+    t = e.tiling()
+    assert t["cx_flux"] == 24 and t["cy_flux"] == 16 and t["cz_flux"] == 12 and 1 <= t["cz_uct"] <= 12
+    assert (t["tile_x"], t["tile_y"]) == (16, 8)

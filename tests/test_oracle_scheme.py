@@ -212,6 +212,51 @@ def test_P7iii_cyclic_axis_covariance():
         assert np.abs(qp[knew] - tr(q[kold])).max() <= 1e-13, (knew, kold)
 
 
+def _mirror(a, axes, stag=None):
+    """Reflection of a periodic array through the planes x_d = 0, d in axes (array axis 2 - d).  Cell-centred
+    data: i -> n-1-i.  A field staggered along `stag` sits at the + face of its cell: x_{i+1/2} -> -x_{i+1/2} is
+    the + face of cell n-2-i, so along that axis the reversed array is rolled by one more cell."""
+    for d in axes:
+        ax = 2 - d
+        a = np.flip(a, ax)
+        if stag == d:
+            a = np.roll(a, -1, ax)
+    return np.ascontiguousarray(a)
+
+
+@pytest.mark.parametrize("axes", [(0,), (1,), (2,), (0, 1, 2)])
+def test_P7iv_reflection_covariance(axes):
+    """The equations are invariant under a mirror reflection (v polar: the components along the reflected axes
+    change sign; B axial: the components along the NON-reflected axes change sign when one axis is reflected, and
+    B is unchanged by the full parity (x,y,z) -> -(x,y,z)), and the scheme, being built from centred INT/DER and
+    from MP5 applied to mirrored stencils for L and R, must be too.  This is what fixes the UCT edge speeds of O7 to
+    a SYMMETRIC function of the two faces adjacent to the edge: taking the speeds of one of them only (or the
+    neighbour on one side only in any upwind formula) breaks the reflection through that axis at O(1) of the
+    dissipative term, while max (and any other symmetric choice) passes."""
+    shape = (16, 12, 10)
+    tb, bf = _turb(shape)
+    f = [tb["rho"], tb["vx"], tb["vy"], tb["vz"], tb["p"]] + bf
+    q, d = _run(shape, f, 3)
+    nref = len(axes)
+    sv = [(-1.0 if c in axes else 1.0) for c in range(3)]                       # polar vector
+    sb = [(-1.0) ** nref * sv[c] for c in range(3)]                            # axial vector: det(R) R
+    fm = [_mirror(f[0], axes)] + [sv[c] * _mirror(f[1 + c], axes) for c in range(3)] + [_mirror(f[4], axes)] + \
+         [sb[c] * _mirror(f[5 + c], axes, stag=c) for c in range(3)]
+    qm, dm = _run(shape, fm, 3)
+    assert dm["t"] == pytest.approx(d["t"], rel=1e-14) and dm["c2p_failures"] == 0
+    assert dm["max_div_b"] < 1e-11
+    exp = {"rho": _mirror(q["rho"], axes), "p": _mirror(q["p"], axes)}
+    for c, k in enumerate(("vx", "vy", "vz")):
+        exp[k] = sv[c] * _mirror(q[k], axes)
+    for c, (kc, kf) in enumerate((("bx", "bxf"), ("by", "byf"), ("bz", "bzf"))):
+        exp[kc] = sb[c] * _mirror(q[kc], axes)
+        exp[kf] = sb[c] * _mirror(q[kf], axes, stag=c)
+    for k, a in exp.items():
+        assert np.abs(qm[k] - a).max() <= 1e-13, (axes, k, np.abs(qm[k] - a).max())
+    # the test has teeth: the fields are not themselves mirror-symmetric
+    assert np.abs(qm["vx"] - q["vx"]).max() > 1e-2
+
+
 def test_rhs_is_flux_difference_and_curl_telescoping():
     """Eq.(9)-(10): the cell sums of rhs(U) and the face sums of rhs(B) vanish identically (periodic)."""
     shape = (12, 10, 8)
