@@ -557,3 +557,27 @@ def test_steps_past_t_end_leave_state_and_failure_count_alone(torch, eb, ob):
     t = e.tiling()
     assert t["cx_flux"] == 24 and t["cy_flux"] == 16 and t["cz_flux"] == 12 and 1 <= t["cz_uct"] <= 12
     assert (t["tile_x"], t["tile_y"]) == (16, 8)
+
+
+def test_con2prim_safeguard_states_agree_with_the_oracle(torch, eb, ob):
+    """The safeguard branch of O2 on the CUDA side: cold ultra-relativistic states (W = 20..40) on which the first
+    Newton step leaves the domain of x(y) (the oracle's instrumented count says for which samples).  echo_con2prim
+    must land on the same root with the same number of iterations (a safeguard step counts as one on both sides)."""
+    n = 50_001
+    s = inputs.random_states(n, seed=777, wmin=20.0, wmax=40.0, log_p_over_rho=(-6.0, -2.0))
+    co = ob.prim2cons(G, *[s[k] for k in "rho vx vy vz p bx by bz".split()])
+    qo = ob.con2prim_trace(G, co["D"], co["Sx"], co["Sy"], co["Sz"], co["U"], s["bx"], s["by"], s["bz"])
+    hit = qo["nsafe"] > 0
+    assert qo["rc"] == 0 and hit.mean() > 0.5
+    qg = eb.con2prim(G, *[dev(torch, co[k]) for k in ("D", "Sx", "Sy", "Sz", "U")], *[dev(torch, s[k]) for k in ("bx", "by", "bz")])
+    it_g = qg["iters"].cpu().numpy()
+    assert (it_g > 0).all()
+    assert np.mean(it_g[hit] != qo["iters"][hit]) < 0.02 and np.mean(it_g != qo["iters"]) < 0.02
+    assert np.abs(it_g - qo["iters"]).max() <= 1
+    eps_w2 = 2.2e-16 * s["W"] ** 2
+    assert (np.abs(qg["rho"].cpu().numpy() / qo["rho"] - 1) <= 100 * eps_w2).all()
+    for k in ("vx", "vy", "vz"):
+        assert absinf(qg[k].cpu().numpy(), qo[k]) <= 1e-13, k
+    assert (np.abs(qg["p"].cpu().numpy() - qo["p"]) <= 5e-15 * co["U"]).all()
+    # and against the true primitives (round trip through the safeguard)
+    assert (np.abs(qg["rho"].cpu().numpy() / s["rho"] - 1) <= 100 * eps_w2).all()

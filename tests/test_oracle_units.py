@@ -314,6 +314,42 @@ def test_con2prim_round_trip_P6():
     assert ep[m].max() <= 1e-12
 
 
+def test_con2prim_safeguard_branch_reaches_the_same_root():
+    """The safeguard of O2 (an iterate with y <= 0 or x(y) outside [0, 1) is replaced by the midpoint with the last
+    valid one).  No state of BJ's P6 range (W <= 10) enters it, but physical states do: for cold ultra-relativistic
+    flows (W = 20..40, p/rho = 1e-6..1e-2) the first Newton step from the upper bound y0 overshoots below the root
+    into x(y) >= 1 for most samples (the instrumented count `nsafe` says which).  What the branch must deliver is
+    fixed by the mathematics, not by the rule: the root is unique, so the primitives must still be the ones the
+    conserved state was built from, to the conditioning of the problem (relative error ~ eps W^2)."""
+    n = 20000
+    s = inputs.random_states(n, seed=777, wmin=20.0, wmax=40.0, log_p_over_rho=(-6.0, -2.0))
+    assert s["W"].min() >= 20.0 - 1e-9 and s["W"].max() <= 40.0 + 1e-9
+    c = ob.prim2cons(G, s["rho"], s["vx"], s["vy"], s["vz"], s["p"], s["bx"], s["by"], s["bz"])
+    r = ob.con2prim_trace(G, c["D"], c["Sx"], c["Sy"], c["Sz"], c["U"], s["bx"], s["by"], s["bz"])
+    hit = r["nsafe"] > 0
+    assert hit.mean() > 0.5, hit.mean()                    # the branch is what this sample exercises
+    assert r["rc"] == 0 and (r["iters"] > 0).all() and r["iters"].max() <= 20
+    assert (r["iters"][hit] >= 3).all()                    # at least: failed step, midpoint, converging step
+    W2 = 1 / np.sqrt(1 - (r["vx"] ** 2 + r["vy"] ** 2 + r["vz"] ** 2))
+    eps_w2 = 2.2e-16 * s["W"] ** 2
+    assert (np.abs(r["rho"] / s["rho"] - 1) <= 60 * eps_w2).all()
+    assert (np.abs(W2 / s["W"] - 1) <= 60 * eps_w2).all()
+    dv = np.sqrt((r["vx"] - s["vx"]) ** 2 + (r["vy"] - s["vy"]) ** 2 + (r["vz"] - s["vz"]) ** 2)
+    assert dv.max() <= 1e-13
+    assert (np.abs(r["p"] - s["p"]) <= 5e-15 * c["U"]).all()
+    # same accuracy whether or not the safeguard was used: it only changes the path to the root
+    e = np.abs(r["rho"] / s["rho"] - 1) / eps_w2
+    assert np.median(e[hit]) < 10 * max(np.median(e[~hit]), 0.05)
+    # and the plain entry point returns the same numbers (the instrumentation changes nothing)
+    r0 = ob.con2prim(G, c["D"], c["Sx"], c["Sy"], c["Sz"], c["U"], s["bx"], s["by"], s["bz"])
+    assert np.array_equal(r0["iters"], r["iters"]) and np.array_equal(r0["rho"], r["rho"]) and np.array_equal(r0["p"], r["p"])
+    # in BJ's own range the branch is never entered (so parity there never depended on it)
+    s6 = inputs.random_states(100000, seed=12345)
+    c6 = ob.prim2cons(G, s6["rho"], s6["vx"], s6["vy"], s6["vz"], s6["p"], s6["bx"], s6["by"], s6["bz"])
+    r6 = ob.con2prim_trace(G, c6["D"], c6["Sx"], c6["Sy"], c6["Sz"], c6["U"], s6["bx"], s6["by"], s6["bz"])
+    assert r6["rc"] == 0 and r6["nsafe"].max() == 0
+
+
 def test_con2prim_flags_unphysical_input():
     r = ob.con2prim(G, [1.0], [0], [0], [0], [-1.0], [0], [0], [0])
     assert r["rc"] != 0 and r["iters"][0] < 0 and np.isnan(r["rho"][0])
