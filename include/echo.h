@@ -223,6 +223,13 @@ int echo_get_tiling(echo_ctx *ctx, int *out);
 /* Kernel classes of the per-kernel timers: 0 k_prim (INT+con2prim), 1..3 k_flux<x,y,z> (REC+HLL+DER+
  * divergence), 4 k_uct, 5 k_update (curl+RK), 6 control kernels, 7 everything else. */
 
+/* Host only.  echo_step replays ONE captured step (its 21 kernels as a CUDA graph, captured at the first call on an
+ * internal stream and launched into the bound stream), which removes the gaps between dependent launches that cost
+ * about a tenth of a step on grids of 32^3-64^3 cells.  enable = 0 makes echo_step launch its kernels one by one
+ * (same kernels, same arguments, bit-identical results); 1 (default) restores the replay.  Plain launches are also
+ * used while echo_timing is on and for the stage-wise entry points. */
+int echo_use_graph(echo_ctx *ctx, int enable);
+
 /* enable != 0: from now on every kernel launch of this handle is bracketed by a CUDA-event pair on
  * the bound stream (no synchronisation, no change to the launch order); also clears the timers and
  * the launch counters.  enable == 0: stops bracketing. */

@@ -46,6 +46,7 @@ SIGNATURES = {
     "echo_stage_sweeps": (_int, [_vp, _int, _dbl]),
     "echo_stage_finish": (_int, [_vp, _int]),
     "echo_get_tiling": (_int, [_vp, C.POINTER(_int)]),
+    "echo_use_graph": (_int, [_vp, _int]),
     "echo_timing": (_int, [_vp, _int]),
     "echo_get_timing": (_int, [_vp, C.POINTER(_dbl), C.POINTER(_long)]),
     "echo_fp64_peak": (_int, [_int, C.POINTER(_dbl), _vp]),
@@ -237,6 +238,10 @@ class Echo:
         self._check(self.L.echo_get_tiling(self.h, out))
         names = ["cx_flux", "cy_flux", "cz_flux", "cz_prim", "cz_uct", "cz_bupd", "tile_x", "tile_y"]
         return dict(zip(names, list(out)))
+
+    def use_graph(self, enable=True):
+        """echo_use_graph: replay one captured step (default) or launch its kernels one by one."""
+        self._check(self.L.echo_use_graph(self.h, 1 if enable else 0))
 
     # ---- measurement aids
     def timing(self, enable=True):

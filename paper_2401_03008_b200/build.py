@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libecho_b200.so")
 SOURCES = ["echo_api.cu"]
-HEADERS = ["echo_kernels.cuh", "echo_uct.cuh", "echo_math.cuh", "echo_types.cuh", os.path.join("..", "..", "include", "echo.h")]
+HEADERS = ["echo_kernels.cuh", "echo_uct.cuh", "echo_math.cuh", "echo_types.cuh", "echo_async.cuh", os.path.join("..", "..", "include", "echo.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]

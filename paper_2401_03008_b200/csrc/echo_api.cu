@@ -1,5 +1,7 @@
 // echo_api.cu — C-ABI layer of libecho_b200 (see include/echo.h): argument checks, workspace
 // carving, kernel launches on the bound stream.  No arithmetic of the method lives here.
+#include <cuda.h>   // CUtensorMap and its enums only: the encoder is fetched through cudaGetDriverEntryPoint
+
 #include <cmath>
 #include <cstddef>
 #include <cstdio>
@@ -27,6 +29,14 @@ struct echo_ctx {
     int rk = 3;              // SSP-RK3 or SSP-RK2 (echo_set_order)
     bool block = false;      // echo_create_block: explicit spacing, halos refreshed by the caller between stages
     bool gate_active = false;   // inside echo_step / echo_stage_*: con2prim failures count only while ctrl->active
+    // one full step captured as a CUDA graph (echo_step replays it)
+    cudaStream_t cap_stream = nullptr;    // capture target (the legacy default stream cannot be captured)
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr;
+    bool capturing = false, graph_failed = false;
+    long graph_launches[ECHO_NKCLASS] = {0};
+    int use_graph = 1;
+    UctMaps uct_maps[2];     // TMA descriptors of the fields k_uct3 stages; [1]: staggered B in the stage buffers
     int device = -1;         // device the bound workspace lives on (echo_bind); every launching call runs there
     // launch configuration of the marching kernels (ensure_tiling; reported by echo_get_tiling)
     struct Tiling { bool ready = false; int cz_prim = 0, cz_uct = 0, cz_bupd = 0, cy_uct_flat = 0, cy_bupd_flat = 0; } til;
@@ -38,7 +48,16 @@ struct echo_ctx {
     size_t ev_used = 0;
     struct Span { int cls; size_t e0, e1; };
     std::vector<Span> spans;
-    ~echo_ctx() { for (cudaEvent_t e : ev_pool) cudaEventDestroy(e); }
+    void drop_graph() {
+        if (gexec) cudaGraphExecDestroy(gexec);
+        if (graph) cudaGraphDestroy(graph);
+        gexec = nullptr; graph = nullptr; graph_failed = false;
+    }
+    ~echo_ctx() {
+        for (cudaEvent_t e : ev_pool) cudaEventDestroy(e);
+        drop_graph();
+        if (cap_stream) cudaStreamDestroy(cap_stream);
+    }
 };
 
 namespace {
@@ -68,10 +87,10 @@ int cuda_fail(echo_ctx *c, cudaError_t e, const char *where) {
 // 256-cell row costs 10 rounds of 32 or 18 of 16, i.e. 320 or 288 row slots for its 261 faces: 0.74 -> 0.71 ms)
 constexpr int FLUX_NT = 128, FLUX_NT_X = 64, FLUX_CMAX = 512;
 
-// Length CZ of the z-chunks of a plane-marching kernel (k_uct2, k_bupd): tiles x chunks blocks run in waves of
+// Length CZ of the z-chunks of a plane-marching kernel (k_uct3, k_bupd): tiles x chunks blocks run in waves of
 // `slots` resident blocks, and every chunk pays about `fill` planes of pipeline fill (window prologue, first copies).
 // Picks the chunk count with the best  (blocks / (waves * slots)) * CZ / (CZ + fill); at 256^3 this is 6 chunks of 43
-// planes for k_uct2 (3072 blocks = 6.9 waves of 444) instead of 3 of 86 (3.5 waves): 1.15 -> 1.08 ms.
+// planes for the UCT kernel (3072 blocks = 6.9 waves of 444) instead of 3 of 86 (3.5 waves): 1.15 -> 1.08 ms.
 int pick_chunk_planes(int tiles, int nz, int slots, int fill) {
     int best_cz = nz;
     double best = -1.0;
@@ -85,13 +104,44 @@ int pick_chunk_planes(int tiles, int nz, int slots, int fill) {
     return best_cz;
 }
 template <typename K>
-int resident_slots(K kernel, int threads) {
+int resident_slots(K kernel, int threads, size_t dyn_smem = 0) {
     int per_sm = 0, sms = 0, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0);
+    if (dyn_smem > 48 * 1024) cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, dyn_smem);
     return std::max(1, per_sm) * std::max(1, sms);
 }
+// ---- TMA descriptors (k_uct3).  A field is a 3-D tensor (nx, ny, nz) of doubles, x fastest; a box is {bx, by, 1}.
+// Encoding needs 16-byte multiples for the row pitch (n_x even) and for the box rows (bx even).
+static_assert(sizeof(TmaDesc) == sizeof(CUtensorMap) && alignof(TmaDesc) >= alignof(CUtensorMap), "TmaDesc mirrors CUtensorMap");
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        cudaGetLastError();
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+bool encode_box(const Grid &g, double *field, int bx, int by, TmaDesc *out) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2]};
+    const cuuint64_t strides[2] = {sizeof(double) * (cuuint64_t)g.n[0], sizeof(double) * (cuuint64_t)g.n[0] * g.n[1]};
+    const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1u}, estr[3] = {1u, 1u, 1u};
+    return enc(reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, field, dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+// maps of stage set `which` (0: staggered B of U^n, 1: of the stage buffers); ok = 0 if the grid has no interior tile
+// or cannot be described (odd n_x): k_uct3 then fills every tile by cp.async
+void build_uct_maps(echo_ctx *c, int which);
 
 enum { KC_PRIM = 0, KC_FLUX = 1, KC_UCT = 4, KC_UPDATE = 5, KC_CTRL = 6, KC_OTHER = 7 };
 
@@ -101,7 +151,9 @@ void ensure_tiling(echo_ctx *c) {
     const Grid &g = c->g;
     const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
     c->til.cz_prim = pick_chunk_planes(tx * ty, g.n[2], resident_slots(k_prim_march<true>, UCT_NT), 2);
-    c->til.cz_uct = pick_chunk_planes(tx * ty, g.n[2], resident_slots(k_uct2<false>, UCT_NT), 3);
+    const int ty3 = (g.n[1] + U3_TY - 1) / U3_TY;
+    c->til.cz_uct = pick_chunk_planes(tx * ty3, g.n[2], resident_slots(k_uct3<false, U3_TY>, U3<U3_TY>::NT, U3<U3_TY>::SMEM), 3);
+    resident_slots(k_uct3<true, U3_TY>, U3<U3_TY>::NT, U3<U3_TY>::SMEM);   // (opts the linear-REC instantiation into its shared memory too)
     c->til.cz_bupd = pick_chunk_planes(tx * ty, g.n[2], resident_slots(k_bupd, UCT_NT), 2);
     c->til.cy_uct_flat = pick_chunk_planes(tx, ty, resident_slots(k_uct2_flat<false>, UCT_NT), 3);
     c->til.cy_bupd_flat = pick_chunk_planes(tx, ty, resident_slots(k_bupd_flat, UCT_NT), 2);
@@ -123,7 +175,7 @@ size_t next_event(echo_ctx *c) {
     return c->ev_used++;
 }
 void tbegin(echo_ctx *c, int cls) {
-    c->launches[cls]++;
+    (c->capturing ? c->graph_launches : c->launches)[cls]++;   // a captured launch runs (and counts) at every replay
     if (c->timing) c->spans.push_back({cls, next_event(c), 0});
 }
 void tend(echo_ctx *c) {
@@ -156,6 +208,28 @@ Stage make_stage(const echo_ctx *c, int which) {
         st.E[d] = c->field[F_E + d];
     }
     return st;
+}
+
+void build_uct_maps(echo_ctx *c, int which) {
+    const Grid &g = c->g;
+    UctMaps &m = c->uct_maps[which];
+    std::memset(&m, 0, sizeof(m));
+    if (g.n[0] % 2 || g.n[0] < 3 * UCT_TX || g.n[1] < 3 * U3_TY || g.n[2] < 2) return;   // no interior tile / unaligned rows
+    const Stage st = make_stage(c, which);
+    double *xr[4] = {st.vb[1][1], const_cast<double *>(st.Bf[1]), st.vb[2][0], const_cast<double *>(st.Bf[2])};
+    double *yr[4] = {st.vb[0][0], const_cast<double *>(st.Bf[0]), st.vb[2][1], const_cast<double *>(st.Bf[2])};
+    bool ok = true;
+    for (int f = 0; f < 4; ++f) {
+        ok = ok && encode_box(g, xr[f], U3_XRP, U3_TY, &m.xr[f]);
+        ok = ok && encode_box(g, yr[f], UCT_TX, U3_TY + 5, &m.yr[f]);
+    }
+    double *sp[3][2] = {{st.ap[0], st.am[0]}, {st.ap[1], st.am[1]}, {st.ap[2], st.am[2]}};
+    for (int f = 0; f < 2; ++f) {
+        ok = ok && encode_box(g, sp[2][f], U3_AP, U3_TY + 1, &m.az[f]);
+        ok = ok && encode_box(g, sp[0][f], UCT_TX, U3_TY + 1, &m.ax[f]);
+        ok = ok && encode_box(g, sp[1][f], U3_AP, U3_TY, &m.ay[f]);
+    }
+    m.ok = ok ? 1 : 0;
 }
 
 // fuse: 0 = plain operator (rhs written), 1 = the z-sweep applies the RK combination of the 5 cell fields
@@ -274,8 +348,6 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
         KL(KC_CTRL, "k_set_dt", k_set_dt<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, ctx->cfl * ctx->hmin));
     }
     {   // plane-marching UCT: 16 x 8 tiles of (x, y), chunks of planes along z sized by pick_chunk_planes
-        // (splitting it into an x/y kernel and a z kernel to shed the z-window registers was measured: 1.28 ms
-        // against 1.21 ms for the single kernel at 256^3, so the single kernel stays)
         if (g.n[2] == 1) {   // 2.5-D: the same kernel marching along y (k_uct2_flat)
             const int tx = (g.n[0] + UCT_TX - 1) / UCT_TX, ty = (g.n[1] + UCT_TY - 1) / UCT_TY;
             ensure_tiling(ctx);
@@ -288,8 +360,11 @@ int launch_uct(echo_ctx *ctx, const Stage &st, bool set_dt) {
         ensure_tiling(ctx);
         const int CZ = ctx->til.cz_uct;
         dim3 grid((g.n[0] + UCT_TX - 1) / UCT_TX, (g.n[1] + UCT_TY - 1) / UCT_TY, (g.n[2] + CZ - 1) / CZ);
-        if (g.rec == 2) KL(KC_UCT, "k_uct2", k_uct2<true><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
-        else KL(KC_UCT, "k_uct2", k_uct2<false><<<grid, UCT_NT, 0, ctx->stream>>>(g, st, CZ));
+        // tiles by TMA where their boxes lie inside the grid, by cp.async along the periodic seams (k_uct3)
+        const UctMaps &maps = ctx->uct_maps[st.Bf[0] == ctx->field[F_BF1] ? 1 : 0];
+        grid.y = (g.n[1] + U3_TY - 1) / U3_TY;
+        if (g.rec == 2) KL(KC_UCT, "k_uct3", k_uct3<true, U3_TY><<<grid, U3<U3_TY>::NT, U3<U3_TY>::SMEM, ctx->stream>>>(g, st, CZ, maps));
+        else KL(KC_UCT, "k_uct3", k_uct3<false, U3_TY><<<grid, U3<U3_TY>::NT, U3<U3_TY>::SMEM, ctx->stream>>>(g, st, CZ, maps));
     }
     return ECHO_OK;
 }
@@ -407,6 +482,7 @@ int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     ctx->device = attr.device;
     DevGuard dev_guard_(ctx);
     ctx->til.ready = false;
+    ctx->drop_graph();
     ctx->ws = static_cast<char *>(dev_workspace);
     ctx->ws_bytes = bytes;
     ctx->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -414,6 +490,8 @@ int echo_bind(echo_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     ctx->part = reinterpret_cast<double *>(ctx->ws + CTRL_BYTES);
     double *f0 = reinterpret_cast<double *>(ctx->ws + CTRL_BYTES + PART_BYTES);
     for (int f = 0; f < NFIELD; ++f) ctx->field[f] = f0 + (size_t)f * ctx->npad;
+    build_uct_maps(ctx, 0);
+    build_uct_maps(ctx, 1);
     Ctrl h;
     std::memset(&h, 0, sizeof(h));
     h.one = 1;
@@ -476,36 +554,25 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
     return ECHO_OK;
 }
 
-int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
-    int rc = check_ready(ctx, true);
-    if (rc) return rc;
-    DevGuard dev_guard_(ctx);
-    if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
-    if (ctx->block && (ctx->g.lo[0] > 0 || ctx->g.lo[1] > 0 || ctx->g.lo[2] > 0))
-        return fail(ctx, ECHO_EINVAL, "a block with halos is stepped stage by stage (echo_stage_sweeps / echo_stage_finish) by its owner");
-    GateScope gate_scope_(ctx);
+// the launches of one full step (t_end comes from the control block)
+static int enqueue_step(echo_ctx *ctx) {
+    int rc;
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     const bool rk2 = ctx->rk == 2;   // SSP-RK2 (O3b): stage 1 as below, then U^{n+1} = 1/2 U^n + 1/2 (U1 + dt L(U1))
+    KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
     if (!ctx->g.uct) {
         // UCT = NO: all 8 fields are cell fields.  Stage 1 writes rhs only; its update is formed by the
         // k_prim of stage 2 (U and B); stages 2 and 3 combine all 8 fields inside their z-sweep.  10 launches.
-        for (int n = 0; n < nsteps; ++n) {
-            KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
-            if ((rc = launch_operator(ctx, s0, 2))) return rc;
-            Stage s12 = s1;
-            for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];
-            const StagePlan p2 = {true, true, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25};
-            if ((rc = launch_operator(ctx, s12, 0, &p2))) return rc;
-            if (!rk2) {
-                const StagePlan p3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
-                if ((rc = launch_operator(ctx, s1, 0, &p3))) return rc;
-            }
-            KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+        if ((rc = launch_operator(ctx, s0, 2))) return rc;
+        Stage s12 = s1;
+        for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];
+        const StagePlan p2 = {true, true, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25};
+        if ((rc = launch_operator(ctx, s12, 0, &p2))) return rc;
+        if (!rk2) {
+            const StagePlan p3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
+            if ((rc = launch_operator(ctx, s1, 0, &p3))) return rc;
         }
-        return ECHO_OK;
-    }
-    for (int n = 0; n < nsteps; ++n) {
-        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+    } else {
         // stage 1: L(U^n), dt from its speeds (S9); B1 = B^n + dt rhs_B now, U1 = U^n + dt rhs_U deferred
         // into the k_prim of stage 2 (st.U = U^n, st.R = rhs, result stored to the stage buffers)
         if ((rc = launch_operator(ctx, s0, 2))) return rc;
@@ -524,8 +591,64 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
             if ((rc = launch_operator(ctx, s1, 0, &pl))) return rc;
             if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false))) return rc;
         }
-        KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
     }
+    KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+    return ECHO_OK;
+}
+
+// Captures enqueue_step once (on an internal stream: the legacy default stream PyTorch hands over cannot be captured)
+// and instantiates it; the executable graph is then launched into the bound stream.  Any failure falls back to plain
+// launches for the rest of the handle's life (graph_failed).
+static bool ensure_graph(echo_ctx *ctx) {
+    if (ctx->gexec) return true;
+    if (ctx->graph_failed) return false;
+    ensure_tiling(ctx);                      // occupancy queries and attribute calls happen before the capture
+    if (!ctx->cap_stream && cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->graph_failed = true;
+        return false;
+    }
+    cudaStream_t user = ctx->stream;
+    for (int c = 0; c < ECHO_NKCLASS; ++c) ctx->graph_launches[c] = 0;
+    bool ok = cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+        ctx->stream = ctx->cap_stream;
+        ctx->capturing = true;
+        const int rc = enqueue_step(ctx);
+        ctx->capturing = false;
+        ctx->stream = user;
+        ok = cudaStreamEndCapture(ctx->cap_stream, &ctx->graph) == cudaSuccess && rc == ECHO_OK && ctx->graph;
+    }
+    ok = ok && cudaGraphInstantiate(&ctx->gexec, ctx->graph, 0) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        ctx->drop_graph();
+        ctx->graph_failed = true;
+    }
+    return ok;
+}
+
+int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
+    int rc = check_ready(ctx, true);
+    if (rc) return rc;
+    DevGuard dev_guard_(ctx);
+    if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
+    if (ctx->block && (ctx->g.lo[0] > 0 || ctx->g.lo[1] > 0 || ctx->g.lo[2] > 0))
+        return fail(ctx, ECHO_EINVAL, "a block with halos is stepped stage by stage (echo_stage_sweeps / echo_stage_finish) by its owner");
+    GateScope gate_scope_(ctx);
+    if (nsteps == 0) return ECHO_OK;
+    KL(KC_CTRL, "k_set_t_end", k_set_t_end<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+    // one captured step replayed nsteps times (no launch gaps between its 21 kernels); plain launches while the
+    // per-kernel timers are on (their event records do not belong in a graph) or if capture is unavailable
+    if (ctx->use_graph && !ctx->timing && ensure_graph(ctx)) {
+        for (int n = 0; n < nsteps; ++n) {
+            CU(cudaGraphLaunch(ctx->gexec, ctx->stream));
+            for (int c = 0; c < ECHO_NKCLASS; ++c) ctx->launches[c] += ctx->graph_launches[c];
+        }
+        return ECHO_OK;
+    }
+    for (int n = 0; n < nsteps; ++n)
+        if ((rc = enqueue_step(ctx))) return rc;
     return ECHO_OK;
 }
 
@@ -811,7 +934,8 @@ int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
     const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
     GateScope gate_scope_(ctx);
     if (stage == 1) {
-        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+        KL(KC_CTRL, "k_set_t_end", k_set_t_end<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
         return launch_sweeps(ctx, s0, 2);
     }
     // stages 2, 3: the stage buffers hold the (halo-refreshed) state; RK combination fused into the z-sweep
@@ -853,6 +977,12 @@ int echo_get_tiling(echo_ctx *ctx, int *out) {
     out[5] = !g.uct ? 0 : (g.n[2] == 1 ? -ctx->til.cy_bupd_flat : ctx->til.cz_bupd);
     out[6] = UCT_TX;
     out[7] = UCT_TY;
+    return ECHO_OK;
+}
+
+int echo_use_graph(echo_ctx *ctx, int enable) {
+    if (!ctx) return ECHO_EINVAL;
+    ctx->use_graph = enable ? 1 : 0;
     return ECHO_OK;
 }
 

@@ -1,11 +1,12 @@
 // echo_kernels.cuh — the kernels of one Runge-Kutta sub-step, sm_100a, FP64.
 //   k_prim      point 1: INT of the staggered B + con2prim                    (a1, a2)
 //   k_flux<D>   points 2+3: REC -> L/R -> HLL flux -> DER + divergence  (a3, a4, a8)
-//   k_uct2      point 4: UCT edge EMFs (echo_uct.cuh, with k_bupd: curl + B update)   (a5, a6)
+//   k_uct3      point 4: UCT edge EMFs (echo_uct.cuh, with k_bupd: curl + B update)   (a5, a6)
 //   k_update    point 4b + 5 (eq.(10)): curl + RK combination of all 8 fields; used for the
 //               unfused stage-1 update of block mode, k_bupd/k_prim<UPD>/k_flux<MODE 1> otherwise   (a6, a7)
 // plus the small control kernels that keep t, dt and a_max on the device.
 #pragma once
+#include "echo_async.cuh"
 #include "echo_math.cuh"
 #include "echo_types.cuh"
 
@@ -27,9 +28,11 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, doub
 }
 
 // ------------------------------------------------------------------ control kernels (1 thread)
-__global__ void k_begin_step(Ctrl *c, double t_end) {
-    c->t_end = t_end;
-    c->active = (c->t < t_end) ? 1 : 0;
+// t_end of the steps that follow (one launch per echo_step call; the steps themselves take no host argument, so that
+// one captured step can be replayed as a CUDA graph)
+__global__ void k_set_t_end(Ctrl *c, double t_end) { c->t_end = t_end; }
+__global__ void k_begin_step(Ctrl *c) {
+    c->active = (c->t < c->t_end) ? 1 : 0;
     c->amax_bits = 0ull;
 }
 __global__ void k_set_dt(Ctrl *c, double cfl_hmin) {
@@ -177,13 +180,6 @@ __global__ void __launch_bounds__(256) k_init(Grid g, const double *rho, const d
 // instructions on the same inputs, hence bit-identically: conservation stays at round-off).
 // REC: the unlimited MP5 value and the S&H test; the limiter proper runs (inline branch) only where
 // the test fires, which on the smooth wave is the couple of cells around each extremum.
-__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void prefetch_l2(const double *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // MODE 0: rhs is written (x) or accumulated (y, z).  MODE 1 (last sweep of RK stages 2 and 3): the
 // completed rhs is consumed at once by the Runge-Kutta combination of the 5 conserved cell fields,
@@ -446,7 +442,7 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
 }
 
 }  // namespace echo
-#include "echo_uct.cuh"   // k_uct2: the plane-marching UCT kernel used by echo_step
+#include "echo_uct.cuh"   // k_uct3: the plane-marching UCT kernel used by echo_step
 namespace echo {
 
 // ------------------------------------------------------------------ points 4b + 5: curl + RK update

@@ -142,7 +142,7 @@ __device__ __forceinline__ double times4(double d) {
 }
 #ifndef ECHO_SH_SUPERSET
 #define ECHO_SH_SUPERSET 1       // sweeps: x 0.785 -> 0.776, y 0.757 -> 0.741, z 0.808 -> 0.804 ms at 256^3
-#define ECHO_SH_SUPERSET_UCT 0   // k_uct2: 1.16 -> 1.19-1.22 ms with it (inline or behind the checked call)
+#define ECHO_SH_SUPERSET_UCT 0   // UCT kernel: 1.16 -> 1.19-1.22 ms with it (inline or behind the checked call)
 #endif
 template <bool INL = true>
 __device__ __forceinline__ void mp5_pair(double s0, double s1, double s2, double s3, double s4, double s5, double &L,
@@ -212,7 +212,7 @@ __device__ __forceinline__ void rec_pair(double s0, double s1, double s2, double
 
 // Branch-free first half of mp5_pair: the two unlimited values and the two S&H test bits (bit 0: L needs the
 // limiter, bit 1: R); mp5_pair_fix applies the limiter afterwards.  Used where several stencils should be
-// interleaved by the compiler before any branch (k_uct2).
+// interleaved by the compiler before any branch (the UCT kernels).
 __device__ __forceinline__ unsigned mp5_pair_fast(double s0, double s1, double s2, double s3, double s4, double s5,
                                                   double &L, double &R) {
     L = (3.0 / 128.0) * s0 + ((-20.0 / 128.0) * s1 + ((90.0 / 128.0) * s2 + ((60.0 / 128.0) * s3 + (-5.0 / 128.0) * s4)));

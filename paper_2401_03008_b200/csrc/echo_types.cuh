@@ -53,6 +53,18 @@ struct Stage {
     double *E[3];          // edge EMFs
 };
 
+// Tensor maps (TMA descriptors, 128 bytes each, built on the host by cuTensorMapEncodeTiled) of the fields the
+// plane-marching UCT kernel stages, one per (field, tile shape); passed by value as a __grid_constant__ parameter.
+struct alignas(64) TmaDesc { unsigned long long w[16]; };     // same size and alignment as CUtensorMap
+struct UctMaps {
+    TmaDesc xr[4];      // vbar_x@y, B_y, vbar_x@z, B_z : boxes 22 x 8   (x0-2 .. x0+19)
+    TmaDesc yr[4];      // vbar_y@x, B_x, vbar_y@z, B_z : boxes 16 x 13  (y0-2 .. y0+10)
+    TmaDesc az[2];      // a+_z, a-_z : 18 x 9
+    TmaDesc ax[2];      // a+_x, a-_x : 16 x 9
+    TmaDesc ay[2];      // a+_y, a-_y : 18 x 8
+    int ok;             // 0: no maps (rows not 16-byte aligned or grid too small): every tile takes the cp.async path
+};
+
 // RK combination  out = c0 * base + c1 * (cur + dt * rhs)   (O9)
 struct Update {
     const double *base[8];   // U^n, Bf^n

@@ -1,18 +1,20 @@
-// echo_uct.cuh — point 4 of a sub-step: the UCT edge EMFs (O7), plane-marching version.
+// echo_uct.cuh — point 4 of a sub-step: the UCT edge EMFs (O7), plane-marching, and the other kernels that
+// march 16 x 8 tiles of (x, y) along z: curl + update of the staggered B (k_bupd), INT + con2prim (k_prim_march).
 //
-// A block owns a TX x TY = 16 x 8 tile of (x, y) and marches along z over a chunk of planes, one
-// plane per round, one cell (three edges) per thread.  What a plane needs:
-//   XR  4 fields reconstructed along x  (vbar_x@y-face, B_y, vbar_x@z-face, B_z): (TX+5) x TY
-//   YR  4 fields reconstructed along y  (vbar_y@x-face, B_x, vbar_y@z-face, B_z): TX x (TY+5)
-//   ZW  4 fields reconstructed along z  (vbar_z@x-face, B_x, vbar_z@y-face, B_y): a 6-plane sliding
-//       window per thread, held in REGISTERS (one new value per field and plane)
-//   AX, AY, AZ  the saved a+/a- of the three directions at the cell and its +1 neighbours along the
-//       two other axes (the edge speed is the max over the two faces adjacent to the edge)
-// XR/YR/AZ of plane k+1 and AX/AY of plane k+2 are brought in by cp.async (LDGSTS) while plane k is
-// computed (double / triple buffers), with the periodic wrap applied to the source coordinates, so
-// every input is read from L2/HBM about once (plus tile halos) and the global-memory latency hides
-// behind the arithmetic.  One __syncthreads per plane.
+// k_uct3: a block owns a TX x TY = 16 x 8 tile of (x, y) and marches along z over a chunk of planes, one plane per
+// round, one cell (three edges) per thread.  What a plane needs:
+//   XR  4 fields reconstructed along x  (vbar_x@y-face, B_y, vbar_x@z-face, B_z): 22 x 8 (x0-2 .. x0+19)
+//   YR  4 fields reconstructed along y  (vbar_y@x-face, B_x, vbar_y@z-face, B_z): 16 x 13 (y0-2 .. y0+10)
+//   ZW  4 fields reconstructed along z  (vbar_z@x-face, B_x, vbar_z@y-face, B_y): a 6-plane sliding window per
+//       thread, held in REGISTERS (one new value per field and plane)
+//   AX, AY, AZ  the saved a+/a- of the three directions at the cell and its +1 neighbours along the two other axes
+//       (the edge speed is the max over the two faces adjacent to the edge)
+// The 14 tiles of a plane form one "package" in shared memory, moved by TMA (tiles inside the grid) or cp.async (tiles
+// on the periodic seams) and completed on an mbarrier; three packages are resident (plane k, the x/y speeds of k+1,
+// and k+2 landing), so every input is read from L2/HBM about once (plus tile halos) and its latency hides behind two
+// planes of arithmetic.
 #pragma once
+#include "echo_async.cuh"
 #include "echo_math.cuh"
 #include "echo_types.cuh"
 
@@ -30,83 +32,156 @@ __device__ __forceinline__ double uct_hll(double ap, double am, double vL, doubl
     return (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) * rcp_fast(ap + am);
 }
 
-// LIN: the limited linear REC of O3b instead of MP5 (echo_set_order)
-template <bool LIN = false>
-__global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
-    __shared__ double sXR[2][4][UCT_XR];
-    __shared__ double sYR[2][4][UCT_YR];
-    __shared__ double sAZ[2][2][UCT_AZ];
-    __shared__ double sAX[3][2][UCT_AX];
-    __shared__ double sAY[3][2][UCT_AY];
+// One upwinded product of O7: MP5 L/R (O3) of (vbar, B) to the edge from the six stencil values p[0], p[S], ...,
+// p[5 S] (vbar) and q[0], ..., q[5 S] (B), then the two-state formula with the edge speeds ap, am.  Shared by the
+// plane-marching kernel (k_uct3) and the flat one (k_uct2_flat), so that the two stay bit-identical.  LIN: the limited linear REC of O3b instead of MP5 (echo_set_order).
+template <bool LIN>
+__device__ __forceinline__ double uct_bracket(const double *p, const double *q, int S, double ap, double am) {
+    double vL, vR, BL, BR;
+    if (LIN) {
+        tvd2_pair(p[S], p[2 * S], p[3 * S], p[4 * S], vL, vR);
+        tvd2_pair(q[S], q[2 * S], q[3 * S], q[4 * S], BL, BR);
+        return uct_hll(ap, am, vL, vR, BL, BR);
+    }
+    const unsigned nv = mp5_pair_fast(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+    const unsigned nb = mp5_pair_fast(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+    if (nv | nb) {
+        mp5_pair_fix(nv, p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
+        mp5_pair_fix(nb, q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
+    }
+    return uct_hll(ap, am, vL, vR, BL, BR);
+}
+
+// ------------------------------------------------------------------ k_uct3: tiles moved by TMA
+// In the round-1 kernel (k_uct2) every thread issued 10-14 eight-byte cp.async per plane, each with its own wrapped
+// source index (a sixth of the kernel's instructions and 40 % of its shared-memory wavefronts,
+// profiles/r1_ncu_full.md).  Here the 14 tiles of a
+// plane (XR, YR: 4 fields each; AZ, AX, AY: 2 each; 19 488 bytes) are 14 TMA box copies (cp.async.bulk.tensor, SASS
+// UTMALDG) issued by ONE thread, completing on one mbarrier by transaction bytes (SASS SYNCS); the other 127
+// threads issue nothing.  A TMA box cannot wrap periodically (out-of-range elements are zero-filled), so only the
+// tiles whose boxes lie inside the grid take this path - at 256^3 that is 82 % of the blocks, at 512^3 91 %; the
+// blocks along the periodic seams of x and y (and every block of a grid without tensor maps: odd n_x, small grids)
+// fill the same shared-memory layout with per-thread 8-byte cp.async copies, which arrive on the same
+// mbarrier (cp.async.mbarrier.arrive.noinc).  z never needs a split: a copy moves one plane, whose index is wrapped
+// by the issuing thread.  The packages of three consecutive planes live in a ring (plane k and the x/y speeds of
+// k+1 are in use while k+2 lands): 57 KB of dynamic shared memory, 3 blocks per SM.
+#ifndef ECHO_UCT_TY
+#define ECHO_UCT_TY 8
+#endif
+constexpr int U3_TY = ECHO_UCT_TY;                                       // tile height of k_uct3 in force
+constexpr int U3_XRP = 22, U3_AP = 18;                                   // row pitches (doubles) of the x-halo tiles
+constexpr int u3_pad16(int n) { return (n + 15) / 16 * 16; }             // tiles start 128-byte aligned (TMA destination)
+// geometry of a plane package for tiles of UCT_TX x TY cells (TY = 8: 4 warps per block; TY = 4: 2 warps)
+template <int TY>
+struct U3 {
+    static constexpr int NT = UCT_TX * TY;                               // threads per block = cells per tile
+    static constexpr int YRH = TY + 5;
+    static constexpr int NXR = U3_XRP * TY, NYR = UCT_TX * YRH;          // elements per field tile
+    static constexpr int NAZ = U3_AP * (TY + 1), NAX = UCT_TX * (TY + 1), NAY = U3_AP * TY;
+    static constexpr int SXR = u3_pad16(NXR), SYR = u3_pad16(NYR), SAZ = u3_pad16(NAZ), SAX = u3_pad16(NAX), SAY = u3_pad16(NAY);
+    static constexpr int XR = 0, YR = XR + 4 * SXR, AZ = YR + 4 * SYR, AX = AZ + 2 * SAZ, AY = AX + 2 * SAX;   // offsets
+    static constexpr int PKG = AY + 2 * SAY;                             // doubles per package (TY = 8: 2464)
+    static constexpr unsigned BYTES = 8u * (4 * NXR + 4 * NYR + 2 * NAZ + 2 * NAX + 2 * NAY);   // bytes that land (19 488)
+    static constexpr int NSLOT = 3;
+    static constexpr size_t SMEM = sizeof(double) * NSLOT * PKG + 128 + 64;
+    static constexpr int NCOPY = (NYR + NT - 1) / NT;                    // cp.async path: elements per thread and region
+};
+
+template <bool LIN = false, int TY = U3_TY>
+__global__ void __launch_bounds__(UCT_TX * TY) k_uct3(Grid g, Stage st, int CZ, const __grid_constant__ UctMaps maps) {
+    using G3 = U3<TY>;
+    constexpr int NT = G3::NT;
+    extern __shared__ __align__(128) unsigned char u3_raw[];
+    double *const pkg = reinterpret_cast<double *>(u3_raw + ((128u - (smem_u32(u3_raw) & 127u)) & 127u));   // [slot][G3::PKG]
+    uint64_t *const full = reinterpret_cast<uint64_t *>(pkg + G3::NSLOT * G3::PKG);  // one barrier per slot
 
     const int tid = threadIdx.x;
     const int tx = tid % UCT_TX, ty = tid / UCT_TX;
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
-    const int x0 = blockIdx.x * UCT_TX, y0 = blockIdx.y * UCT_TY, z0 = blockIdx.z * CZ;
+    const int x0 = blockIdx.x * UCT_TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * CZ;
     const int CZv = min(CZ, nz - z0);
     const int sy = g.s[1], sz = g.s[2];
+    // all 14 boxes inside the grid?  (block-uniform)
+    const bool tma = maps.ok && x0 >= 2 && x0 + UCT_TX + 4 <= nx && y0 >= 2 && y0 + TY + 3 <= ny;
 
-    // in-plane source offsets of the (at most two) elements this thread copies per region
-    int oXR[2], oYR[2], oAX[2], oAY[2], oAZ[2];
+    // cp.async path (seam tiles): in-plane source offsets of the (at most two) elements this thread copies per region
+    int oXR[G3::NCOPY], oYR[G3::NCOPY], oAX[G3::NCOPY], oAY[G3::NCOPY], oAZ[G3::NCOPY];
+    if (!tma) {
 #pragma unroll
-    for (int it = 0; it < 2; ++it) {
-        const int e = tid + UCT_NT * it;
-        oXR[it] = (e < UCT_XR) ? wrapi(x0 - 2 + e % UCT_XRW, nx) + sy * wrapi(y0 + e / UCT_XRW, ny) : -1;
-        oYR[it] = (e < UCT_YR) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 - 2 + e / UCT_TX, ny) : -1;
-        oAX[it] = (e < UCT_AX) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 + e / UCT_TX, ny) : -1;
-        oAY[it] = (e < UCT_AY) ? wrapi(x0 + e % UCT_AYW, nx) + sy * wrapi(y0 + e / UCT_AYW, ny) : -1;
-        oAZ[it] = (e < UCT_AZ) ? wrapi(x0 + e % UCT_AYW, nx) + sy * wrapi(y0 + e / UCT_AYW, ny) : -1;
+        for (int it = 0; it < G3::NCOPY; ++it) {
+            const int e = tid + NT * it;
+            oXR[it] = (e < G3::NXR) ? wrapi(x0 - 2 + e % U3_XRP, nx) + sy * wrapi(y0 + e / U3_XRP, ny) : -1;
+            oYR[it] = (e < G3::NYR) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 - 2 + e / UCT_TX, ny) : -1;
+            oAX[it] = (e < G3::NAX) ? wrapi(x0 + e % UCT_TX, nx) + sy * wrapi(y0 + e / UCT_TX, ny) : -1;
+            oAY[it] = (e < G3::NAY) ? wrapi(x0 + e % U3_AP, nx) + sy * wrapi(y0 + e / U3_AP, ny) : -1;
+            oAZ[it] = (e < G3::NAZ) ? wrapi(x0 + e % U3_AP, nx) + sy * wrapi(y0 + e / U3_AP, ny) : -1;
+        }
     }
     // XR = {vbar_x@y, B_y, vbar_x@z, B_z}; YR = {vbar_y@x, B_x, vbar_y@z, B_z}; ZW = {vbar_z@x, B_x, vbar_z@y, B_y}
-    // (direction d saves vbar_{(d+1)%3} in slot 0 and vbar_{(d+2)%3} in slot 1)
     const double *fXR[4] = {st.vb[1][1], st.Bf[1], st.vb[2][0], st.Bf[2]};
     const double *fYR[4] = {st.vb[0][0], st.Bf[0], st.vb[2][1], st.Bf[2]};
     const double *fZW[4] = {st.vb[0][1], st.Bf[0], st.vb[1][0], st.Bf[1]};
 
-    auto issue_plane = [&](int k, int slot) {          // XR, YR, AZ of plane k
-        const int pz = sz * wrapi(k, nz);
+    auto issue_package = [&](int k, int slot) {            // all tiles of plane k into ring slot `slot`
+        const int kz = wrapi(k, nz);
+        double *base = pkg + slot * G3::PKG;
+        if (tma) {
+            if (tid == 0) {
+                mbar_arrive_expect_tx(&full[slot], G3::BYTES);
 #pragma unroll
-        for (int it = 0; it < 2; ++it) {
-            const int e = tid + UCT_NT * it;
-            if (oXR[it] >= 0) {
+                for (int f = 0; f < 4; ++f) tma_load_3d(base + G3::XR + f * G3::SXR, &maps.xr[f], x0 - 2, y0, kz, &full[slot]);
 #pragma unroll
-                for (int f = 0; f < 4; ++f) cp_async8(&sXR[slot][f][e], fXR[f] + (pz + oXR[it]));
-            }
-            if (oYR[it] >= 0) {
+                for (int f = 0; f < 4; ++f) tma_load_3d(base + G3::YR + f * G3::SYR, &maps.yr[f], x0, y0 - 2, kz, &full[slot]);
 #pragma unroll
-                for (int f = 0; f < 4; ++f) cp_async8(&sYR[slot][f][e], fYR[f] + (pz + oYR[it]));
+                for (int f = 0; f < 2; ++f) {
+                    tma_load_3d(base + G3::AZ + f * G3::SAZ, &maps.az[f], x0, y0, kz, &full[slot]);
+                    tma_load_3d(base + G3::AX + f * G3::SAX, &maps.ax[f], x0, y0, kz, &full[slot]);
+                    tma_load_3d(base + G3::AY + f * G3::SAY, &maps.ay[f], x0, y0, kz, &full[slot]);
+                }
             }
-            if (oAZ[it] >= 0) {
-                cp_async8(&sAZ[slot][0][e], st.ap[2] + (pz + oAZ[it]));
-                cp_async8(&sAZ[slot][1][e], st.am[2] + (pz + oAZ[it]));
-            }
-        }
-    };
-    auto issue_speeds = [&](int k, int slot) {         // AX, AY of plane k
-        const int pz = sz * wrapi(k, nz);
+        } else {
+            const int pz = sz * kz;
 #pragma unroll
-        for (int it = 0; it < 2; ++it) {
-            const int e = tid + UCT_NT * it;
-            if (oAX[it] >= 0) {
-                cp_async8(&sAX[slot][0][e], st.ap[0] + (pz + oAX[it]));
-                cp_async8(&sAX[slot][1][e], st.am[0] + (pz + oAX[it]));
+            for (int it = 0; it < G3::NCOPY; ++it) {
+                const int e = tid + NT * it;
+                if (oXR[it] >= 0) {
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) cp_async8(base + G3::XR + f * G3::SXR + e, fXR[f] + (pz + oXR[it]));
+                }
+                if (oYR[it] >= 0) {
+#pragma unroll
+                    for (int f = 0; f < 4; ++f) cp_async8(base + G3::YR + f * G3::SYR + e, fYR[f] + (pz + oYR[it]));
+                }
+                if (oAZ[it] >= 0) {
+                    cp_async8(base + G3::AZ + e, st.ap[2] + (pz + oAZ[it]));
+                    cp_async8(base + G3::AZ + G3::SAZ + e, st.am[2] + (pz + oAZ[it]));
+                }
+                if (oAX[it] >= 0) {
+                    cp_async8(base + G3::AX + e, st.ap[0] + (pz + oAX[it]));
+                    cp_async8(base + G3::AX + G3::SAX + e, st.am[0] + (pz + oAX[it]));
+                }
+                if (oAY[it] >= 0) {
+                    cp_async8(base + G3::AY + e, st.ap[1] + (pz + oAY[it]));
+                    cp_async8(base + G3::AY + G3::SAY + e, st.am[1] + (pz + oAY[it]));
+                }
             }
-            if (oAY[it] >= 0) {
-                cp_async8(&sAY[slot][0][e], st.ap[1] + (pz + oAY[it]));
-                cp_async8(&sAY[slot][1][e], st.am[1] + (pz + oAY[it]));
-            }
+            cp_async_arrive_on(&full[slot]);               // this thread's share of the package has landed
         }
     };
 
-    // this thread's cell column (clamped for the loads of ragged tiles; stores are masked)
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < G3::NSLOT; ++s) mbar_init(&full[s], tma ? 1u : (unsigned)NT);
+        mbar_init_fence();
+    }
+    __syncthreads();
+
     const bool cellok = (x0 + tx < nx) && (y0 + ty < ny);
     const int ccol = min(x0 + tx, nx - 1) + sy * min(y0 + ty, ny - 1);
 
-    // prologue: plane z0 (+ speeds of z0 and z0+1) by cp.async; z-window planes z0-2 .. z0+3 directly
-    issue_plane(z0, 0);
-    issue_speeds(z0, 0);
-    issue_speeds(z0 + 1, 1);
-    cp_async_commit();
+    // prologue: packages of planes z0 and z0+1; z-window planes z0-2 .. z0+3 directly
+    issue_package(z0, 0);
+    issue_package(z0 + 1, 1);
     double zw[4][6];
 #pragma unroll
     for (int m = 0; m < 6; ++m) {
@@ -115,74 +190,59 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
         for (int f = 0; f < 4; ++f) zw[f][m] = __ldg(fZW[f] + (pz + ccol));
     }
 
+    int s0 = 0;                                            // ring slot of plane k
     for (int r = 0; r < CZv; ++r) {
         const int k = z0 + r;
-        cp_async_wait_all();
-        __syncthreads();
-        const bool more = (r + 1 < CZv);
-        double znew[4] = {0.0, 0.0, 0.0, 0.0};
-        if (more) {
-            issue_plane(k + 1, (r + 1) & 1);
-            issue_speeds(k + 2, (r + 2) % 3);
-            cp_async_commit();
+        const int s1 = (s0 + 1 == G3::NSLOT) ? 0 : s0 + 1, s2 = (s1 + 1 == G3::NSLOT) ? 0 : s1 + 1;
+        // plane z0 + r is the (r / 3)-th package of its slot: the parity of that phase
+        mbar_wait(&full[s0], (unsigned)((r / G3::NSLOT) & 1));
+        mbar_wait(&full[s1], (unsigned)(((r + 1) / G3::NSLOT) & 1));
+        __syncthreads();                                   // every warp is through plane k-1: its slot (s2) is free
+        if (r + 2 <= CZv) issue_package(k + 2, s2);        // (plane z0+CZv only lends its x/y speeds to the last plane)
+        double znew[4];
+        {
             const int pz = sz * wrapi(k + 4, nz);
 #pragma unroll
             for (int f = 0; f < 4; ++f) znew[f] = __ldg(fZW[f] + (pz + ccol));
         }
 
         if (cellok) {
-            const int ps = r & 1, as0 = r % 3, as1 = (r + 1) % 3;
-            // saved speeds at the cell and its +1 neighbours
-            const int iax = ty * UCT_TX + tx, iay = ty * UCT_AYW + tx;
-            const double axp = sAX[as0][0][iax], axm = sAX[as0][1][iax];
-            const double ayp = sAY[as0][0][iay], aym = sAY[as0][1][iay];
-            const double azp = sAZ[ps][0][iay], azm = sAZ[ps][1][iay];
-            // one upwinded product at a time: MP5 L/R (O3) of (vbar, B) to the edge, then O7
-            auto bracket = [&](const double *p, const double *q, int S, double ap, double am) {
-                double vL, vR, BL, BR;
-                if (LIN) {
-                    tvd2_pair(p[S], p[2 * S], p[3 * S], p[4 * S], vL, vR);
-                    tvd2_pair(q[S], q[2 * S], q[3 * S], q[4 * S], BL, BR);
-                    return uct_hll(ap, am, vL, vR, BL, BR);
-                }
-                const unsigned nv = mp5_pair_fast(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
-                const unsigned nb = mp5_pair_fast(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
-                if (nv | nb) {
-                    mp5_pair_fix(nv, p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
-                    mp5_pair_fix(nb, q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
-                }
-                return uct_hll(ap, am, vL, vR, BL, BR);
-            };
+            const double *P0 = pkg + s0 * G3::PKG, *P1 = pkg + s1 * G3::PKG;
+            const int ixr = ty * U3_XRP + tx, iyr = ty * UCT_TX + tx, iax = ty * UCT_TX + tx, iay = ty * U3_AP + tx;
+            const double *AX0 = P0 + G3::AX, *AY0 = P0 + G3::AY, *AZ0 = P0 + G3::AZ, *AX1 = P1 + G3::AX, *AY1 = P1 + G3::AY;
+            const double axp = AX0[iax], axm = AX0[G3::SAX + iax];
+            const double ayp = AY0[iay], aym = AY0[G3::SAY + iay];
+            const double azp = AZ0[iay], azm = AZ0[G3::SAZ + iay];
             auto along_x = [&](int f, double ap, double am) {
-                const double *p = &sXR[ps][f][ty * UCT_XRW + tx];
-                return bracket(p, p + UCT_XR, 1, ap, am);
+                const double *p = P0 + G3::XR + f * G3::SXR + ixr;
+                return uct_bracket<LIN>(p, p + G3::SXR, 1, ap, am);
             };
             auto along_y = [&](int f, double ap, double am) {
-                const double *p = &sYR[ps][f][ty * UCT_TX + tx];
-                return bracket(p, p + UCT_YR, UCT_TX, ap, am);
+                const double *p = P0 + G3::YR + f * G3::SYR + iyr;
+                return uct_bracket<LIN>(p, p + G3::SYR, UCT_TX, ap, am);
             };
-            auto along_z = [&](int f, double ap, double am) { return bracket(zw[f], zw[f + 1], 1, ap, am); };
+            auto along_z = [&](int f, double ap, double am) { return uct_bracket<LIN>(zw[f], zw[f + 1], 1, ap, am); };
             // E_z: i = x, j = y
-            const double ez = -along_x(0, dmax(axp, sAX[as0][0][iax + UCT_TX]), dmax(axm, sAX[as0][1][iax + UCT_TX])) +
-                              along_y(0, dmax(ayp, sAY[as0][0][iay + 1]), dmax(aym, sAY[as0][1][iay + 1]));
+            const double ez = -along_x(0, dmax(axp, AX0[iax + UCT_TX]), dmax(axm, AX0[G3::SAX + iax + UCT_TX])) +
+                              along_y(0, dmax(ayp, AY0[iay + 1]), dmax(aym, AY0[G3::SAY + iay + 1]));
             // E_y: i = z, j = x
-            const double ey = -along_z(0, dmax(azp, sAZ[ps][0][iay + 1]), dmax(azm, sAZ[ps][1][iay + 1])) +
-                              along_x(2, dmax(axp, sAX[as1][0][iax]), dmax(axm, sAX[as1][1][iax]));
+            const double ey = -along_z(0, dmax(azp, AZ0[iay + 1]), dmax(azm, AZ0[G3::SAZ + iay + 1])) +
+                              along_x(2, dmax(axp, AX1[iax]), dmax(axm, AX1[G3::SAX + iax]));
             // E_x: i = y, j = z
-            const double ex = -along_y(2, dmax(ayp, sAY[as1][0][iay]), dmax(aym, sAY[as1][1][iay])) +
-                              along_z(2, dmax(azp, sAZ[ps][0][iay + UCT_AYW]), dmax(azm, sAZ[ps][1][iay + UCT_AYW]));
+            const double ex = -along_y(2, dmax(ayp, AY1[iay]), dmax(aym, AY1[G3::SAY + iay])) +
+                              along_z(2, dmax(azp, AZ0[iay + U3_AP]), dmax(azm, AZ0[G3::SAZ + iay + U3_AP]));
             const int o = sz * k + ccol;
             st.E[0][o] = ex;
             st.E[1][o] = ey;
             st.E[2][o] = ez;
         }
-        // slide the z-window
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
 #pragma unroll
             for (int m = 0; m < 5; ++m) zw[f][m] = zw[f][m + 1];
             zw[f][5] = znew[f];
         }
+        s0 = s1;
     }
 }
 
@@ -190,7 +250,7 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2(Grid g, Stage st, int CZ) {
 
 // ------------------------------------------------------------------ points 4b + 5 for the staggered B
 // k_bupd: curl of the DER-corrected edge EMFs (O8, eq.(10)) and the Runge-Kutta combination of the
-// three face fields (O9), plane-marching like k_uct2: the x- and y-stencils of a plane come from
+// three face fields (O9), plane-marching like k_uct3: the x- and y-stencils of a plane come from
 // cp.async-fed tiles (one plane ahead), the z-stencils from a 6-plane register window, the old B values
 // of the next plane are loaded one round early.  Pure streaming: 12 doubles per cell.
 //   dB_x/dt = -[D_y E_z - D_z E_y],  dB_y/dt = -[D_z E_x - D_x E_z],  dB_z/dt = -[D_x E_y - D_y E_x]
@@ -306,7 +366,7 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const
 // for it, compute and exit.  k_uct2_flat / k_bupd_flat run the same arithmetic with the roles of "plane" taken by
 // consecutive (x, y) tiles along y: the tiles of y-tile t+1 arrive by cp.async while tile t is computed.  Through the
 // periodic wrap the six z-stencil values of a cell are all the cell's own value and plane k+1 is plane k, so the
-// z-brackets see six equal values (the generic arithmetic applied to them: bitwise what k_uct2 / k_bupd give on a
+// z-brackets see six equal values (the generic arithmetic applied to them: bitwise what k_uct3 / k_bupd give on a
 // one-plane grid, and what a thicker grid with z-independent data gives - the dimensional-reduction tests).
 namespace echo {
 
@@ -397,19 +457,7 @@ __global__ void __launch_bounds__(UCT_NT) k_uct2_flat(Grid g, Stage st, int CY) 
             const double ayp = sAY[ps][0][iay], aym = sAY[ps][1][iay];
             const double azp = sAZ[ps][0][iay], azm = sAZ[ps][1][iay];
             auto bracket = [&](const double *p, const double *q, int S, double ap, double am) {
-                double vL, vR, BL, BR;
-                if (LIN) {
-                    tvd2_pair(p[S], p[2 * S], p[3 * S], p[4 * S], vL, vR);
-                    tvd2_pair(q[S], q[2 * S], q[3 * S], q[4 * S], BL, BR);
-                    return uct_hll(ap, am, vL, vR, BL, BR);
-                }
-                const unsigned nv = mp5_pair_fast(p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
-                const unsigned nb = mp5_pair_fast(q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
-                if (nv | nb) {
-                    mp5_pair_fix(nv, p[0], p[S], p[2 * S], p[3 * S], p[4 * S], p[5 * S], vL, vR);
-                    mp5_pair_fix(nb, q[0], q[S], q[2 * S], q[3 * S], q[4 * S], q[5 * S], BL, BR);
-                }
-                return uct_hll(ap, am, vL, vR, BL, BR);
+                return uct_bracket<LIN>(p, q, S, ap, am);
             };
             auto along_x = [&](int f, double ap, double am) {
                 const double *p = &sXR[ps][f][ty * UCT_XRW + tx];

@@ -581,3 +581,26 @@ def test_con2prim_safeguard_states_agree_with_the_oracle(torch, eb, ob):
     assert (np.abs(qg["p"].cpu().numpy() - qo["p"]) <= 5e-15 * co["U"]).all()
     # and against the true primitives (round trip through the safeguard)
     assert (np.abs(qg["rho"].cpu().numpy() / s["rho"] - 1) <= 100 * eps_w2).all()
+
+
+def test_graph_replay_equals_plain_launches_bitwise(torch, eb, ob):
+    """echo_step replays one captured step as a CUDA graph; with echo_use_graph(0) it launches the same kernels one by
+    one.  Same kernels, same arguments: the two must agree in every bit, including a clipped last step, steps past
+    t_end, and a second echo_step call that re-uses the instantiated graph with another t_end."""
+    shape = (40, 24, 20)
+    w = turb_inputs(torch, eb, ob, None, shape=shape)
+    outs = []
+    for graph in (True, False):
+        e = eb.Echo(*shape, G, 0.3)
+        e.use_graph(graph)
+        e.set_primitives(*[dev(torch, w[k]) for k in SETK])
+        e.step(3)
+        t3 = e.diagnostics()["t"]
+        e.step(4, t3 * 1.9)                  # 2 full steps + a clipped one + a no-op
+        d = e.diagnostics()
+        assert d["steps"] == 6 and d["t"] == t3 * 1.9 and d["c2p_failures"] == 0
+        q = e.get_primitives()
+        outs.append([q[k].clone() for k in PRIMS + ["bxf", "byf", "bzf"]] + [d["dt_last"]])
+    for a, b in zip(outs[0][:-1], outs[1][:-1]):
+        assert torch.equal(a, b)
+    assert outs[0][-1] == outs[1][-1]
