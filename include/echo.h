@@ -63,7 +63,7 @@ int echo_set_scheme(echo_ctx *ctx, int uct, int ho);
  * MC(a, b) = minmod(2a, 2b, (a+b)/2) (reading O3b), used by the sweeps and by UCT; built with the
  * second-order INT/DER only: ECHO_EINVAL unless echo_set_scheme(ctx, uct, 0) was called first.
  * rk = 3: SSP-RK3 (default); rk = 2: U1 = U^n + dt L(U^n), U^{n+1} = (U^n + U1 + dt L(U1))/2, dt as for RK3.
- * Block handles (echo_create_block) accept (5, 3) only.  ECHO_EINVAL on other values, ECHO_ESTATE once a state exists. */
+ * ECHO_EINVAL on other values, ECHO_ESTATE once a state exists. */
 int echo_set_order(echo_ctx *ctx, int rec, int rk);
 
 /* Host only.  Frees the handle (never the workspace). */
@@ -190,8 +190,9 @@ int echo_diagnostics(echo_ctx *ctx, double *out);
  *     for stage in 1, 2, 3:
  *         echo_stage_sweeps(ctx, stage, t_end)      INT + con2prim + the three sweeps (+ a_max in stage 1)
  *         [stage 1: all-reduce(max) of the 8-byte a_max word at echo_ctrl_offset(0) across the blocks]
- *         echo_stage_finish(ctx, stage)             (stage 1: dt) UCT, update of the stage's output fields
- *         [refresh the halos of fields 8..15 (stages 1, 2) or 0..7 (stage 3) from the neighbours]
+ *         echo_stage_finish(ctx, stage)             (stage 1: dt) UCT, update of the staggered B
+ *         [refresh the halos of the 8 fields echo_stage_halo_fields names from the neighbours: packed messages,
+ *          echo_halo_pack / echo_halo_unpack; the 5 cell fields may already travel while echo_stage_finish runs]
  * echo_set_primitives / echo_get_primitives work on the padded block as on a plain box. */
 echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, int gnx, int gny, int gnz,
                             int halo_x, int halo_y, int halo_z);
@@ -205,9 +206,31 @@ size_t echo_field_offset(const echo_ctx *ctx, int field);
  * 3 = con2prim failure count (uint64). */
 size_t echo_ctrl_offset(int what);
 
-/* First and second half of RK stage `stage` (1..3) of a block step; see above.  No synchronisation. */
+/* First and second half of RK stage `stage` (1 .. 3, or 1 .. 2 with SSP-RK2) of a block step; see above.  These are the
+ * halves echo_step itself is made of (same kernels, same arguments), so a decomposed run repeats the undecomposed one
+ * bit for bit.  No synchronisation.  ECHO_EINVAL on a uct = 0 handle. */
 int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end);
 int echo_stage_finish(echo_ctx *ctx, int stage);
+
+/* Host only.  fields (HOST, 8 ints) = the workspace fields whose halos the NEXT half needs from the neighbouring
+ * blocks once stage `stage` has finished: five cell fields then three face fields.  After stage 1 these are the rhs of
+ * the cell fields (24..28: the update U1 = U^n + dt rhs is formed inside the INT + con2prim pass of stage 2, for every
+ * cell of the padded block, from the refreshed rhs) and the stage B (13..15); after an inner stage the stage state
+ * (8..15); after the last stage the state (0..7).  The five cell fields are final when echo_stage_sweeps returns, the
+ * three face fields when echo_stage_finish does - so the exchange of the former can overlap the UCT kernels. */
+int echo_stage_halo_fields(const echo_ctx *ctx, int stage, int *fields);
+
+/* Packed halo messages of a block handle: ONE buffer per axis and side holds the slabs of 8 fields, [field][cell of the
+ * slab, x fastest], each slab halo_d cells thick along `axis` and spanning the whole padded block along the other two
+ * axes (edges and corners travel with the later axes when the axes are exchanged in the order x, y, z).
+ * echo_halo_doubles: doubles per message (0 if the axis is not decomposed).  echo_halo_pack gathers the INTERIOR slab
+ * next to side (0 = low, 1 = high) - what the neighbour on that side needs - into buf; echo_halo_unpack scatters buf
+ * into the HALO on that side.  fields: HOST array of 8 field indices (echo_stage_halo_fields; -1 = leave that slot
+ * of the message alone, so that the cell fields and the face fields of a stage can travel separately); buf: DEVICE;
+ * cuda_stream: the stream to run on (NULL = the bound stream).  One kernel per call, no synchronisation. */
+size_t echo_halo_doubles(const echo_ctx *ctx, int axis);
+int echo_halo_pack(echo_ctx *ctx, const int *fields, int axis, int side, double *buf, void *cuda_stream);
+int echo_halo_unpack(echo_ctx *ctx, const int *fields, int axis, int side, const double *buf, void *cuda_stream);
 
 /* Host only (needs the device of the bound workspace for the occupancy query).  The launch configuration in force
  * for this handle, for tests that place samples across tile seams: out (HOST, 8 ints) = {cells per chunk of the

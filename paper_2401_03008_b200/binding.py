@@ -45,6 +45,10 @@ SIGNATURES = {
     "echo_ctrl_offset": (_sz, [_int]),
     "echo_stage_sweeps": (_int, [_vp, _int, _dbl]),
     "echo_stage_finish": (_int, [_vp, _int]),
+    "echo_stage_halo_fields": (_int, [_vp, _int, C.POINTER(_int)]),
+    "echo_halo_doubles": (_sz, [_vp, _int]),
+    "echo_halo_pack": (_int, [_vp, C.POINTER(_int), _int, _int, _vp, _vp]),
+    "echo_halo_unpack": (_int, [_vp, C.POINTER(_int), _int, _int, _vp, _vp]),
     "echo_get_tiling": (_int, [_vp, C.POINTER(_int)]),
     "echo_use_graph": (_int, [_vp, _int]),
     "echo_timing": (_int, [_vp, _int]),
@@ -238,6 +242,24 @@ class Echo:
         self._check(self.L.echo_get_tiling(self.h, out))
         names = ["cx_flux", "cy_flux", "cz_flux", "cz_prim", "cz_uct", "cz_bupd", "tile_x", "tile_y"]
         return dict(zip(names, list(out)))
+
+    def stage_halo_fields(self, stage):
+        """The 8 workspace fields whose halos the next half needs after stage `stage` (5 cell fields, 3 face fields)."""
+        out = (_int * 8)()
+        self._check(self.L.echo_stage_halo_fields(self.h, int(stage), out))
+        return list(out)
+
+    def halo_doubles(self, axis):
+        return int(self.L.echo_halo_doubles(self.h, int(axis)))
+
+    def halo_pack(self, fields, axis, side, buf, stream=None):
+        """Gathers the interior slabs next to `side` of the 8 `fields` into the FP64 CUDA tensor buf (one kernel)."""
+        arr = (_int * 8)(*[int(f) for f in fields])
+        self._check(self.L.echo_halo_pack(self.h, arr, int(axis), int(side), _dev(buf, self.halo_doubles(axis)), stream))
+
+    def halo_unpack(self, fields, axis, side, buf, stream=None):
+        arr = (_int * 8)(*[int(f) for f in fields])
+        self._check(self.L.echo_halo_unpack(self.h, arr, int(axis), int(side), _dev(buf, self.halo_doubles(axis)), stream))
 
     def use_graph(self, enable=True):
         """echo_use_graph: replay one captured step (default) or launch its kernels one by one."""

@@ -554,15 +554,62 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
     return ECHO_OK;
 }
 
+// The UCT = YES step as six halves: stage_sweeps(s) = points 1-3 of sub-step s, stage_finish(s) = point 4
+// + the staggered part of point 5.  echo_step runs them back to back; a domain-decomposed run
+// (echo_stage_sweeps / echo_stage_finish) runs the SAME halves with a halo refresh after each finish, so the two
+// execute the same kernels with the same arguments.  rk2: SSP-RK2 (O3b) ends after stage 2 with weights 1/2, 1/2.
+//   stage 1: L(U^n), dt from its speeds (S9); B1 = B^n + dt rhs_B now, U1 = U^n + dt rhs_U DEFERRED into the k_prim of
+//            stage 2 (st.U = U^n, st.R = rhs, result stored to the stage buffers) - so what the next stage needs
+//            from the neighbours after stage 1 is the rhs of the cell fields and B1 (stage_halo_fields)
+//   stage 2: U2 = 3/4 U^n + 1/4 (U1 + dt L(U1)); the cell fields are combined inside the z-sweep
+//   stage 3: U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
+static int stage_sweeps_impl(echo_ctx *ctx, int stage) {
+    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    const bool rk2 = ctx->rk == 2;
+    if (stage == 1) {
+        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+        return launch_sweeps(ctx, s0, 2);
+    }
+    if (stage == 2) {
+        Stage s12 = s1;                                   // operator state: faces from the stage buffers ...
+        for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];   // ... cell fields = U^n (+ dt R inside k_prim)
+        const StagePlan pl = {true, true, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25};
+        return launch_sweeps(ctx, s12, 0, &pl);
+    }
+    const StagePlan pl = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
+    return launch_sweeps(ctx, s1, 0, &pl);
+}
+static int stage_finish_impl(echo_ctx *ctx, int stage) {
+    int rc;
+    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    const bool rk2 = ctx->rk == 2;
+    if (stage == 1) {
+        if ((rc = launch_uct(ctx, s0, true))) return rc;
+        return launch_update(ctx, s0, 0, 1, 0.0, 1.0, false);
+    }
+    if ((rc = launch_uct(ctx, s1, false))) return rc;
+    if (stage == 2) rc = launch_update(ctx, s1, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25, false);
+    else rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false);
+    if (rc) return rc;
+    if (stage == ctx->rk) KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+    return ECHO_OK;
+}
+// the fields whose halos the next half needs from the neighbouring blocks after stage `stage` (8 field indices)
+static void stage_halo_fields(const echo_ctx *ctx, int stage, int *f) {
+    const bool last = stage == ctx->rk;
+    for (int v = 0; v < 5; ++v) f[v] = (stage == 1 ? F_R : last ? F_U : F_U1) + v;
+    for (int d = 0; d < 3; ++d) f[5 + d] = (last ? F_BF : F_BF1) + d;
+}
+
 // the launches of one full step (t_end comes from the control block)
 static int enqueue_step(echo_ctx *ctx) {
     int rc;
-    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
-    const bool rk2 = ctx->rk == 2;   // SSP-RK2 (O3b): stage 1 as below, then U^{n+1} = 1/2 U^n + 1/2 (U1 + dt L(U1))
-    KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
     if (!ctx->g.uct) {
         // UCT = NO: all 8 fields are cell fields.  Stage 1 writes rhs only; its update is formed by the
         // k_prim of stage 2 (U and B); stages 2 and 3 combine all 8 fields inside their z-sweep.  10 launches.
+        const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+        const bool rk2 = ctx->rk == 2;
+        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
         if ((rc = launch_operator(ctx, s0, 2))) return rc;
         Stage s12 = s1;
         for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];
@@ -572,27 +619,13 @@ static int enqueue_step(echo_ctx *ctx) {
             const StagePlan p3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
             if ((rc = launch_operator(ctx, s1, 0, &p3))) return rc;
         }
-    } else {
-        // stage 1: L(U^n), dt from its speeds (S9); B1 = B^n + dt rhs_B now, U1 = U^n + dt rhs_U deferred
-        // into the k_prim of stage 2 (st.U = U^n, st.R = rhs, result stored to the stage buffers)
-        if ((rc = launch_operator(ctx, s0, 2))) return rc;
-        if ((rc = launch_update(ctx, s0, 0, 1, 0.0, 1.0, false))) return rc;
-        // stage 2: U2 = 3/4 U^n + 1/4 (U1 + dt L(U1)); the cell fields are combined inside the z-sweep
-        {
-            Stage s12 = s1;                       // operator state: faces from the stage buffers ...
-            for (int v = 0; v < 5; ++v) s12.U[v] = s0.U[v];   // ... cell fields = U^n (+ dt R inside k_prim)
-            const StagePlan pl = {true, true, 1, rk2 ? 0 : 1, rk2 ? 0.5 : 0.75, rk2 ? 0.5 : 0.25};
-            if ((rc = launch_operator(ctx, s12, 0, &pl))) return rc;
-            if ((rc = launch_update(ctx, s1, 1, rk2 ? 0 : 1, pl.c0, pl.c1, false))) return rc;
-        }
-        // stage 3: U^{n+1} = 1/3 U^n + 2/3 (U2 + dt L(U2))
-        if (!rk2) {
-            const StagePlan pl = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
-            if ((rc = launch_operator(ctx, s1, 0, &pl))) return rc;
-            if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false))) return rc;
-        }
+        KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+        return ECHO_OK;
     }
-    KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+    for (int stage = 1; stage <= ctx->rk; ++stage) {
+        if ((rc = stage_sweeps_impl(ctx, stage))) return rc;
+        if ((rc = stage_finish_impl(ctx, stage))) return rc;
+    }
     return ECHO_OK;
 }
 
@@ -892,7 +925,6 @@ int echo_set_order(echo_ctx *ctx, int rec, int rk) {
     if (!ctx) return ECHO_EINVAL;
     if (ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_order must precede echo_set_primitives");
     if ((rec != 5 && rec != 2) || (rk != 3 && rk != 2)) return fail(ctx, ECHO_EINVAL, "rec must be 5 or 2, rk 3 or 2");
-    if (ctx->block && (rec != 5 || rk != 3)) return fail(ctx, ECHO_EINVAL, "block handles run MP5 + SSP-RK3 only");
     if (rec == 2 && ctx->g.ho)
         return fail(ctx, ECHO_EINVAL, "linear reconstruction is built with the second-order INT/DER: echo_set_scheme(ctx, uct, 0) first");
     ctx->g.rec = rec;
@@ -929,38 +961,75 @@ int echo_stage_sweeps(echo_ctx *ctx, int stage, double t_end) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     DevGuard dev_guard_(ctx);
-    if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
-    if (!ctx->g.uct || ctx->rk != 3) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES and SSP-RK3 only");
-    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
+    if (!ctx->g.uct) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES only");
+    if (stage < 1 || stage > ctx->rk) return fail(ctx, ECHO_EINVAL, "stage must be 1 .. number of RK stages");
     GateScope gate_scope_(ctx);
-    if (stage == 1) {
-        KL(KC_CTRL, "k_set_t_end", k_set_t_end<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
-        KL(KC_CTRL, "k_begin_step", k_begin_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
-        return launch_sweeps(ctx, s0, 2);
-    }
-    // stages 2, 3: the stage buffers hold the (halo-refreshed) state; RK combination fused into the z-sweep
-    const StagePlan pl2 = {false, true, 1, 1, 0.75, 0.25}, pl3 = {false, true, 1, 0, 1.0 / 3.0, 2.0 / 3.0};
-    return launch_sweeps(ctx, s1, 0, stage == 2 ? &pl2 : &pl3);
+    if (stage == 1) KL(KC_CTRL, "k_set_t_end", k_set_t_end<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
+    return stage_sweeps_impl(ctx, stage);
 }
 
 int echo_stage_finish(echo_ctx *ctx, int stage) {
     int rc = check_ready(ctx, true);
     if (rc) return rc;
     DevGuard dev_guard_(ctx);
-    if (stage < 1 || stage > 3) return fail(ctx, ECHO_EINVAL, "stage must be 1, 2 or 3");
-    if (!ctx->g.uct || ctx->rk != 3) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES and SSP-RK3 only");
-    const Stage s0 = make_stage(ctx, 0), s1 = make_stage(ctx, 1);
-    if (stage == 1) {
-        // dt from the (all-reduced) a_max, UCT, then the UNFUSED update of all 8 fields: U1 must exist in
-        // memory for the halo refresh that precedes stage 2
-        if ((rc = launch_uct(ctx, s0, true))) return rc;
-        return launch_update(ctx, s0, 0, 1, 0.0, 1.0, true);
-    }
-    if ((rc = launch_uct(ctx, s1, false))) return rc;
-    if (stage == 2) return launch_update(ctx, s1, 1, 1, 0.75, 0.25, false);
-    if ((rc = launch_update(ctx, s1, 1, 0, 1.0 / 3.0, 2.0 / 3.0, false))) return rc;
-    KL(KC_CTRL, "k_end_step", k_end_step<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
+    if (!ctx->g.uct) return fail(ctx, ECHO_EINVAL, "the stage-wise entry points are built for UCT=YES only");
+    if (stage < 1 || stage > ctx->rk) return fail(ctx, ECHO_EINVAL, "stage must be 1 .. number of RK stages");
+    GateScope gate_scope_(ctx);
+    return stage_finish_impl(ctx, stage);
+}
+
+int echo_stage_halo_fields(const echo_ctx *ctx, int stage, int *fields) {
+    if (!ctx || !fields || stage < 1 || stage > ctx->rk || !ctx->g.uct) return ECHO_EINVAL;
+    stage_halo_fields(ctx, stage, fields);
     return ECHO_OK;
+}
+
+// ---- packed halo slabs: all 8 fields of one side of one axis in ONE message
+static int halo_slab(const echo_ctx *ctx, int axis, int side, bool interior, int *start, int *width) {
+    if (axis < 0 || axis > 2 || side < 0 || side > 1) return ECHO_EINVAL;
+    const Grid &g = ctx->g;
+    const int h = g.lo[axis];
+    if (h <= 0) return ECHO_EINVAL;                       // this axis is not decomposed
+    *width = h;
+    // interior slab next to `side` (what the neighbour on that side needs) or the halo on that side
+    *start = side == 0 ? (interior ? h : 0) : (interior ? g.n[axis] - 2 * h : g.n[axis] - h);
+    return ECHO_OK;
+}
+
+size_t echo_halo_doubles(const echo_ctx *ctx, int axis) {
+    if (!ctx || axis < 0 || axis > 2 || ctx->g.lo[axis] <= 0) return 0;
+    return (size_t)8 * ctx->g.lo[axis] * (size_t)(ctx->g.N / ctx->g.n[axis]);
+}
+
+static int halo_copy(echo_ctx *ctx, const int *fields, int axis, int side, double *buf, void *cuda_stream, bool pack) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    DevGuard dev_guard_(ctx);
+    if (!fields || !buf) return fail(ctx, ECHO_EINVAL, "null argument");
+    int start = 0, width = 0;
+    if ((rc = halo_slab(ctx, axis, side, pack, &start, &width))) return fail(ctx, rc, "axis is not decomposed or bad axis / side");
+    HaloFields hf;
+    for (int v = 0; v < 8; ++v) {
+        if (fields[v] < -1 || fields[v] >= NFIELD) return fail(ctx, ECHO_EINVAL, "field index out of range");
+        hf.f[v] = fields[v] < 0 ? nullptr : ctx->field[fields[v]];   // -1: this slot of the message is skipped
+    }
+    const Grid &g = ctx->g;
+    const long long per_field = (long long)width * (g.N / g.n[axis]);
+    cudaStream_t st = cuda_stream ? static_cast<cudaStream_t>(cuda_stream) : ctx->stream;
+    const int blocks = (int)std::min<long long>((per_field + 255) / 256, 148LL * 32);
+    cudaStream_t bound = ctx->stream;
+    ctx->stream = st;                                     // (the timers, if on, bracket on the stream that runs the copy)
+    if (pack) KL(KC_OTHER, "k_halo_pack", k_halo_copy<true><<<dim3(blocks, 8), 256, 0, st>>>(g, hf, buf, axis, start, width, per_field));
+    else KL(KC_OTHER, "k_halo_unpack", k_halo_copy<false><<<dim3(blocks, 8), 256, 0, st>>>(g, hf, buf, axis, start, width, per_field));
+    ctx->stream = bound;
+    return ECHO_OK;
+}
+
+int echo_halo_pack(echo_ctx *ctx, const int *fields, int axis, int side, double *buf, void *cuda_stream) {
+    return halo_copy(ctx, fields, axis, side, buf, cuda_stream, true);
+}
+int echo_halo_unpack(echo_ctx *ctx, const int *fields, int axis, int side, const double *buf, void *cuda_stream) {
+    return halo_copy(ctx, fields, axis, side, const_cast<double *>(buf), cuda_stream, false);
 }
 
 int echo_get_tiling(echo_ctx *ctx, int *out) {

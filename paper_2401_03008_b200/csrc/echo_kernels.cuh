@@ -553,6 +553,31 @@ __global__ void __launch_bounds__(256) k_divb(Grid g, const double *B0, const do
     if (tid == 0) atomic_max_nonneg((unsigned long long *)blockmax, sm[0]);
 }
 
+// ------------------------------------------------------------------ packed halo slabs (domain decomposition)
+// One launch moves the slab  start <= c_axis < start + width  (full extent along the other two axes) of 8 fields
+// between the padded block and one contiguous message buffer laid out [field][slab cell, x fastest]:
+// PACK = true gathers (block -> buffer), false scatters (buffer -> block).  blockIdx.y = field.
+struct HaloFields { double *f[8]; };
+template <bool PACK>
+__global__ void __launch_bounds__(256) k_halo_copy(Grid g, HaloFields hf, double *buf, int axis, int start, int width,
+                                                   long long per_field) {
+    int d[3] = {g.n[0], g.n[1], g.n[2]};
+    d[axis] = width;
+    double *fld = hf.f[blockIdx.y];
+    if (!fld) return;                                   // skipped slot of the message
+    double *msg = buf + per_field * blockIdx.y;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < per_field; t += (long long)gridDim.x * blockDim.x) {
+        int c[3];
+        c[0] = (int)(t % d[0]);
+        c[1] = (int)((t / d[0]) % d[1]);
+        c[2] = (int)(t / ((long long)d[0] * d[1]));
+        c[axis] += start;
+        const long long cell = c[0] + (long long)g.s[1] * c[1] + (long long)g.s[2] * c[2];
+        if (PACK) msg[t] = fld[cell];
+        else fld[cell] = msg[t];
+    }
+}
+
 // ------------------------------------------------------------------ deterministic reductions
 // NPART contiguous chunks; each block sums its chunk with a fixed tree, the host adds the NPART
 // partials in extended precision.  rows 0..7: sums of the 8 evolved fields.

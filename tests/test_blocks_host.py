@@ -1,5 +1,7 @@
-"""CPU checks of the multi-rank plumbing of row (f1): the decomposition bookkeeping and the halo exchange over
-torch.distributed with the gloo backend (world sizes 2 and 4), on plain CPU tensors."""
+"""CPU checks of the multi-rank plumbing of row (f1): the decomposition bookkeeping and the PACKED halo exchange
+(blocks.exchange_packed: one message per axis and side for all fields, sent in a cell part and a face part) over
+torch.distributed with the gloo backend (world sizes 2 and 4), on plain CPU tensors with the torch reference
+pack / unpack (the CUDA pack kernels are compared with these in tests/test_gpu_blocks.py)."""
 import json
 import os
 import subprocess
@@ -33,8 +35,23 @@ for a in glob:
             lo, _, _, hi = blocks.slabs(t, axis)
             lo.fill_(float("nan")); hi.fill_(float("nan"))
     ts.append(t)
-blocks.exchange_halos(ts, d, rank, dist)
-ok = all(np.array_equal(t.numpy(), d.cut(rank, a)) for t, a in zip(ts, glob))
+# packed messages: 8 slots per buffer (5 "cell" + 3 "face"), sent in two parts as RankBlock does; slots 0-4 and
+# 5-7 carry the same two tensors over and over, a skipped slot (None) must leave its part of the message alone
+def per(axis):
+    n = list(d.local); n[axis] = blocks.HALO
+    return n[0] * n[1] * n[2]
+bufs = [tuple(torch.full((8 * per(ax),), -7.0, dtype=torch.float64) for _ in range(4)) if d.p[ax] > 1 else None for ax in range(3)]
+cells = [ts[0], ts[1], ts[0], ts[1], ts[0], None, None, None]
+faces = [None] * 5 + [ts[1], ts[0], ts[1]]
+for tensors, part in ((cells, blocks.CELLS), (faces, blocks.FACES)):
+    blocks.exchange_packed(d, rank, dist, bufs,
+                           lambda ax, side, buf: blocks.pack_slabs(tensors, ax, side, buf),
+                           lambda ax, side, buf: blocks.unpack_slabs(tensors, ax, side, buf),
+                           part=lambda ax: slice(part.start * per(ax), part.stop * per(ax)))
+    if part is blocks.CELLS:      # after the first part every halo is already restored (both tensors travelled)
+        ok_first = all(np.array_equal(t.numpy(), d.cut(rank, a)) for t, a in zip(ts, glob))
+ok = ok_first and all(np.array_equal(t.numpy(), d.cut(rank, a)) for t, a in zip(ts, glob))
+assert blocks._masked(list(range(8)), blocks.FACES) == [-1] * 5 + [5, 6, 7]
 # a_max style all-reduce of a bit pattern
 w = torch.tensor([np.float64(0.1 * (rank + 1)).view(np.int64)], dtype=torch.int64)
 dist.all_reduce(w, op=dist.ReduceOp.MAX)

@@ -1,7 +1,8 @@
-"""Row (f1): the domain-decomposed step (one padded periodic block per rank, halo refresh of the 8 evolved fields
-after every RK stage, all-reduce(max) of a_max) against the undecomposed run of the same library.  All blocks
-live in this process on one GPU (LocalBlocks): the same kernels, the same arithmetic per cell and an exact max,
-so the interiors must agree BIT FOR BIT; a wrong halo width, slab, corner or reduction shows up at once."""
+"""Row (f1): the domain-decomposed step (one padded periodic block per rank, packed halo refresh of 8 fields after
+every RK stage, all-reduce(max) of a_max) against the undecomposed run of the same library.  All blocks live in
+this process on one GPU (LocalBlocks): the stage halves are the ones echo_step is made of, the same arithmetic
+per cell and an exact max, so the interiors must agree BIT FOR BIT; a wrong halo width, slab, corner, field list
+or reduction shows up at once."""
 import numpy as np
 import pytest
 
@@ -12,8 +13,41 @@ G = 4.0 / 3.0
 SETK = "rho vx vy vz p bxf byf bzf".split()
 
 
-@pytest.mark.parametrize("p", [(2, 1, 1), (1, 2, 2), (2, 2, 2), (1, 1, 3)])
-def test_blocks_match_single_domain_bitwise(p):
+def test_pack_kernels_equal_the_torch_reference():
+    """echo_halo_pack / echo_halo_unpack against blocks.pack_slabs / unpack_slabs (the form the gloo test runs),
+    for every axis and side, with skipped slots."""
+    import torch
+    from paper_2401_03008_b200 import binding as eb, blocks
+    e = eb.Echo(40, 24, 32, G, 0.3, block=(64, 24, 64, 8, 0, 8))
+    g = torch.Generator(device="cuda").manual_seed(3)
+    fields = [24, 25, 26, -1, 28, 13, -1, 15]
+    for f in range(44):
+        e.field(f).copy_(torch.randn(e.shape, generator=g, device="cuda", dtype=torch.float64))
+    tens = [e.field(f) if f >= 0 else None for f in fields]
+    assert e.halo_doubles(1) == 0 and e.halo_doubles(0) == 8 * 8 * 24 * 32 and e.halo_doubles(2) == 8 * 8 * 40 * 24
+    for axis in (0, 2):
+        for side in (0, 1):
+            a = torch.full((e.halo_doubles(axis),), -7.0, dtype=torch.float64, device="cuda")
+            b = a.clone()
+            e.halo_pack(fields, axis, side, a)
+            blocks.pack_slabs(tens, axis, side, b)
+            assert torch.equal(a, b), (axis, side)
+            assert (a.view(8, -1)[3] == -7.0).all()                  # skipped slot untouched
+            before = [e.field(f).clone() for f in range(44)]
+            msg = torch.randn(e.halo_doubles(axis), generator=g, device="cuda", dtype=torch.float64)
+            ref = [t.clone() for t in before]
+            blocks.unpack_slabs([ref[f] if f >= 0 else None for f in fields], axis, side, msg)
+            e.halo_unpack(fields, axis, side, msg)
+            for f in range(44):
+                assert torch.equal(e.field(f), ref[f]), (axis, side, f)
+    assert e.L.echo_halo_pack(e.h, (eb.C.c_int * 8)(*[0] * 8), 1, 0, a.data_ptr(), None) == eb.ECHO_EINVAL   # y is not decomposed
+    assert e.stage_halo_fields(1) == [24, 25, 26, 27, 28, 13, 14, 15]
+    assert e.stage_halo_fields(2) == list(range(8, 16)) and e.stage_halo_fields(3) == list(range(8))
+
+
+@pytest.mark.parametrize("p,order", [((2, 1, 1), (5, 3)), ((1, 2, 2), (5, 3)), ((2, 2, 2), (5, 3)), ((1, 1, 3), (5, 3)),
+                                     ((2, 1, 2), (2, 2))])
+def test_blocks_match_single_domain_bitwise(p, order):
     import torch
     from paper_2401_03008_b200 import binding as eb, blocks
     from oracle import binding as ob
@@ -22,9 +56,10 @@ def test_blocks_match_single_domain_bitwise(p):
     w = inputs.turbulence(None, shape=gn)
     bo = ob.faces_from_potential(w["ax"], w["ay"], w["az"])
     w["bxf"], w["byf"], w["bzf"] = [b + w["b0"][d] for d, b in enumerate(bo)]
-    e = eb.Echo(*gn, G, 0.3)
+    rec, rk = order                        # (2, 2): linear REC + SSP-RK2 with the second-order INT/DER
+    e = eb.Echo(*gn, G, 0.3, ho=(rec == 5), rec=rec, rk=rk)
     e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
-    lb = blocks.LocalBlocks(gn, p, G, 0.3)
+    lb = blocks.LocalBlocks(gn, p, G, 0.3, ho=(rec == 5), rec=rec, rk=rk)
     lb.set_primitives(w)
     t_end = 2.5 * 0.3 / 48 / 0.9          # inside the third step: exercises the clipped dt on every block
     e.step(4, t_end)
