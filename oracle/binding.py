@@ -37,6 +37,8 @@ def lib():
         L = C.CDLL(build())
         L.oracle_create.restype = C.c_void_p
         L.oracle_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.oracle_create_bounded.restype = C.c_void_p
+        L.oracle_create_bounded.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _ip, _ip]
         L.oracle_destroy.argtypes = [C.c_void_p]
         L.oracle_destroy.restype = None
         L.oracle_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
@@ -88,14 +90,24 @@ DIAG_NAMES = ["t", "dt_last", "steps", "amax", "sum_D", "sum_Sx", "sum_Sy", "sum
 class Oracle:
     """One periodic unit box.  Arrays are numpy float64 of shape (nz, ny, nx) (x fastest)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, uct=True, ho=True, rec=5, rk=3):
+    def __init__(self, nx, ny, nz, gamma, cfl, uct=True, ho=True, rec=5, rk=3, boundaries=None, gn=None):
         """uct / ho: the paper's scheme switches.  With uct=False the three B arrays given to
         set_primitives (and returned as bxf, byf, bzf) are CELL-CENTRED.  rec / rk: 5 / 3 = MP5 + SSP-RK3 (default),
-        2 / 2 = limited linear reconstruction + SSP-RK2."""
+        2 / 2 = limited linear reconstruction + SSP-RK2.
+        boundaries = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi) with 0 periodic, 1 reflecting, 2 outflow (row f4): nx, ny, nz
+        are then the INTERIOR cells and every array has 8 ghost layers on each side of a bounded axis; gn = (gnx, gny,
+        gnz): the spacing is h_d = 1/gn_d (default gn = n: the interior is the unit box)."""
         self.L = lib()
-        self.shape = (nz, ny, nx)
         self.n = (nx, ny, nz)
-        self.h = self.L.oracle_create(nx, ny, nz, gamma, cfl)
+        if boundaries is None:
+            self.ng = (0, 0, 0)
+            self.h = self.L.oracle_create(nx, ny, nz, gamma, cfl)
+        else:
+            kinds = (C.c_int * 6)(*[int(k) for k in boundaries])
+            self.ng = tuple(8 if boundaries[2 * a] else 0 for a in range(3))
+            gnp = (C.c_int * 3)(*[int(v) for v in gn]) if gn is not None else None
+            self.h = self.L.oracle_create_bounded(nx, ny, nz, gamma, cfl, kinds, gnp)
+        self.shape = (nz + 2 * self.ng[2], ny + 2 * self.ng[1], nx + 2 * self.ng[0])
         if not self.h:
             raise ValueError("oracle_create: bad arguments")
         if not (uct and ho):
@@ -112,6 +124,10 @@ class Oracle:
 
     def _new(self, k):
         return [np.empty(self.shape, dtype=np.float64) for _ in range(k)]
+
+    def interior(self):
+        """Slices (z, y, x) of the interior cells of a bounded grid's arrays."""
+        return tuple(slice(g, s - g) for g, s in zip(self.ng[::-1], self.shape))
 
     def set_primitives(self, rho, vx, vy, vz, p, bxf, byf, bzf):
         arrs = [_c(a) for a in (rho, vx, vy, vz, p, bxf, byf, bzf)]

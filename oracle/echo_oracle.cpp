@@ -26,6 +26,12 @@
 // other conserved variables, with no divergence control ("the magnetic field is not staggered but it is
 // treated as the other cell-centered variables").
 //
+// Non-periodic boundaries ("next" row f4, first slice; the paper's production runs are periodic, its code has
+// ghost cells filled before every stencil loop): oracle_create_bounded pads the grid with NG = 8
+// ghost cells on each side of every bounded axis (the dependency reach of one sub-step) and refills them before every
+// evaluation of L(U) - reflecting wall (mirror image with the parity of each field under the reflection) or
+// zero-gradient outflow (copy of the nearest interior value).  DESIGN.md section 12.
+//
 // Pins (tests/test_oracle_*.py): see the list in DESIGN.md §"Oracle pins".
 // parity unpinned: inside the MP5 limiter branch, the published design constants 1/2 (v^MD), 4/3 (v^LC) and 4
 // (inside d^M4) against nearby values.  The paper prints nothing that fixes them; what IS pinned about the branch
@@ -338,7 +344,72 @@ struct Ctx {
     long steps = 0;
     Stats c2p;  // statistics of the most recent full-domain con2prim pass
     long c2p_fail_total = 0;
+    // non-periodic boundaries: ghost width per axis (0 = periodic) and kind per (axis, side): 1 reflecting, 2 outflow
+    int ng[3] = {0, 0, 0};
+    int bc[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+    bool interior(const int c[3]) const {
+        for (int d = 0; d < 3; ++d)
+            if (c[d] < ng[d] || c[d] >= g.n[d] - ng[d]) return false;
+        return true;
+    }
+    // d-faces of the interior: entry c is the face on the + side of cell c, so along d the low wall face (entry
+    // ng - 1) belongs to it as well
+    bool interior_face(const int c[3], int d) const {
+        for (int a = 0; a < 3; ++a) {
+            const int lo = (a == d && ng[a]) ? ng[a] - 1 : ng[a];
+            if (c[a] < lo || c[a] >= g.n[a] - ng[a]) return false;
+        }
+        return true;
+    }
 };
+
+// Ghost fill of the evolved fields of a bounded grid (state or, equally, its rhs: the rules are linear).  Along a
+// bounded axis a with interior cells lo <= c_a < hi, ghost layer m = 0 .. NG-1:
+//   cell-centred along a (D, S, U and the two transverse B components):
+//        low:  ghost lo-1-m  <-  interior lo+m        high: ghost hi+m  <-  interior hi-1-m        (reflecting)
+//        low:  ghost lo-1-m  <-  interior lo          high: ghost hi+m  <-  interior hi-1          (outflow)
+//   B_a itself is staggered along a (entry c = face on the + side of cell c): the wall faces lo-1 and hi-1 are evolved,
+//        low:  face lo-1-m   <-  face lo-1+m (m >= 1)  high: face hi-1+m <-  face hi-1-m (m >= 1)   (reflecting)
+//        low:  face lo-1-m   <-  face lo-1   (m >= 1)  high: face hi-1+m <-  face hi-1   (m >= 1)   (outflow)
+// Reflecting parity (the mirror symmetry of the equations, pinned for the periodic scheme by P7iv): scalars D, U even;
+// the momentum component normal to the wall odd, the tangential ones even (polar vector); B_a even, the tangential B
+// components odd (axial vector).  Axes are filled in the order x, y, z over the full padded extent of the other axes,
+// so edges and corners get the composition of the two (three) rules.
+void fill_ghosts(const Ctx &cx, Field U[5], Field Bf[3]) {
+    const Grid &g = cx.g;
+    for (int a = 0; a < 3; ++a) {
+        const int NG = cx.ng[a];
+        if (!NG) continue;
+        const int lo = NG, hi = g.n[a] - NG;
+        for (int side = 0; side < 2; ++side) {
+            const int kind = cx.bc[a][side];
+            FOR_CELLS(g, c) {
+                CELL(c);
+                const int ca = c[a];
+                const bool ghost = side == 0 ? ca < lo : ca >= hi;
+                if (!ghost) continue;
+                const int m = side == 0 ? lo - 1 - ca : ca - hi;          // ghost layer 0 .. NG-1
+                int src[3] = {c[0], c[1], c[2]};
+                const long dst = g.idx(c[0], c[1], c[2]);
+                // cell-centred fields
+                src[a] = kind == 1 ? (side == 0 ? lo + m : hi - 1 - m) : (side == 0 ? lo : hi - 1);
+                const long sc = g.idx(src[0], src[1], src[2]);
+                for (int v = 0; v < 5; ++v) {
+                    const double sgn = (kind == 1 && v == 1 + a) ? -1.0 : 1.0;   // normal momentum is odd
+                    U[v][dst] = sgn * U[v][sc];
+                }
+                for (int b = 0; b < 3; ++b)
+                    if (b != a) Bf[b][dst] = (kind == 1 ? -1.0 : 1.0) * Bf[b][sc];   // tangential B is odd
+                // the normal B: faces; the wall face (low side: entry lo-1) is not a ghost
+                const int mf = side == 0 ? lo - 1 - ca : ca - (hi - 1);   // distance of this face from the wall face
+                if (mf >= 1) {
+                    src[a] = kind == 1 ? (side == 0 ? lo - 1 + mf : hi - 1 - mf) : (side == 0 ? lo - 1 : hi - 1);
+                    Bf[a][dst] = Bf[a][g.idx(src[0], src[1], src[2])];
+                }
+            }
+        }
+    }
+}
 
 // Step 1 of a sub-step: INT of the staggered B to centres, then con2prim everywhere.
 void centre_b(const Grid &g, const Field Bf[3], Field Bc[3], int ho = 1) {
@@ -359,12 +430,15 @@ void primitives(const Ctx &cx, const State &s, Field P[5], Field Bc[3], Stats &s
     else for (int d = 0; d < 3; ++d) Bc[d] = s.Bf[d];   // UCT=NO: the evolved field is already cell-centred
     for (int v = 0; v < 5; ++v) P[v].assign(g.N, 0.0);
     st = Stats();
-    for (long c = 0; c < g.N; ++c) {
+    FOR_CELLS(g, cc) {
+        CELL(cc);
+        const long c = g.idx(cc[0], cc[1], cc[2]);
         const double u[5] = {s.U[0][c], s.U[1][c], s.U[2][c], s.U[3][c], s.U[4][c]};
         const double B[3] = {Bc[0][c], Bc[1][c], Bc[2][c]};
         double q[5];
         const int it = con2prim(cx.gam, u, B, q);
         for (int v = 0; v < 5; ++v) P[v][c] = q[v];
+        if (!cx.interior(cc)) continue;   // ghost cells of a bounded grid: inverted, but not part of the statistics
         ++st.calls;
         if (it < 0) ++st.fails;
         const int ai = it < 0 ? -it : it;
@@ -435,7 +509,7 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
             am[d][i0] = ex[1];
             vbar[d][0][i0] = ex[2];
             vbar[d][1][i0] = ex[3];
-            amax = std::fmax(amax, std::fmax(ex[0], ex[1]));  // point 5
+            if (cx.interior_face(c, d)) amax = std::fmax(amax, std::fmax(ex[0], ex[1]));  // point 5
         }
     }
     r.amax = amax;
@@ -524,6 +598,7 @@ void compute_rhs(Ctx &cx, const State &s, Rhs &r) {
 void rk3_step(Ctx &cx, double t_end) {
     const Grid &g = cx.g;
     State &s = cx.s;
+    fill_ghosts(cx, s.U, s.Bf);          // (bounded grids only; no-op on a periodic box)
     State s0 = s;
     Rhs r;
     compute_rhs(cx, s, r);
@@ -535,11 +610,13 @@ void rk3_step(Ctx &cx, double t_end) {
         for (int v = 0; v < 5; ++v) s.U[v][c] = s0.U[v][c] + dt * r.U[v][c];
         for (int v = 0; v < 3; ++v) s.Bf[v][c] = s0.Bf[v][c] + dt * r.B[v][c];
     }
+    fill_ghosts(cx, s.U, s.Bf);
     compute_rhs(cx, s, r);
     for (long c = 0; c < g.N; ++c) {
         for (int v = 0; v < 5; ++v) s.U[v][c] = 0.75 * s0.U[v][c] + 0.25 * (s.U[v][c] + dt * r.U[v][c]);
         for (int v = 0; v < 3; ++v) s.Bf[v][c] = 0.75 * s0.Bf[v][c] + 0.25 * (s.Bf[v][c] + dt * r.B[v][c]);
     }
+    fill_ghosts(cx, s.U, s.Bf);
     compute_rhs(cx, s, r);
     for (long c = 0; c < g.N; ++c) {
         for (int v = 0; v < 5; ++v)
@@ -547,6 +624,7 @@ void rk3_step(Ctx &cx, double t_end) {
         for (int v = 0; v < 3; ++v)
             s.Bf[v][c] = (1.0 / 3.0) * s0.Bf[v][c] + (2.0 / 3.0) * (s.Bf[v][c] + dt * r.B[v][c]);
     }
+    fill_ghosts(cx, s.U, s.Bf);
     cx.t += dt;
     cx.dt_last = dt;
     ++cx.steps;
@@ -645,6 +723,36 @@ void *oracle_create(int nx, int ny, int nz, double gamma, double cfl) {
 
 void oracle_destroy(void *h) { delete static_cast<Ctx *>(h); }
 
+// Bounded grid (row f4): nx, ny, nz INTERIOR cells with the spacing h_d = 1/gn_d of a unit box of gn cells (gn = NULL:
+// gn_d = n_d, the interior IS the unit box); kinds[2 a + side] = 0 periodic axis
+// (both sides), 1 reflecting wall, 2 zero-gradient outflow.  Every array passed in or out then has n_d + 16 entries
+// along a bounded axis (8 ghost layers on each side); ghost entries given to oracle_set_primitives are ignored
+// except the normal B at the low wall face (entry 7 of that axis).  UCT=HO=YES, MP5, RK3 only.
+void *oracle_create_bounded(int nx, int ny, int nz, double gamma, double cfl, const int *kinds, const int *gn) {
+    if (nx < 1 || ny < 1 || nz < 1 || !(gamma > 1.0) || !(cfl > 0.0) || !kinds) return nullptr;
+    const int n[3] = {nx, ny, nz};
+    int ng[3];
+    for (int a = 0; a < 3; ++a) {
+        const int k0 = kinds[2 * a], k1 = kinds[2 * a + 1];
+        if ((k0 == 0) != (k1 == 0) || k0 < 0 || k0 > 2 || k1 < 0 || k1 > 2) return nullptr;
+        ng[a] = k0 ? 8 : 0;
+        if (ng[a] && n[a] < 8) return nullptr;
+    }
+    Ctx *cx = new Ctx();
+    cx->g = make_grid(nx + 2 * ng[0], ny + 2 * ng[1], nz + 2 * ng[2]);
+    for (int a = 0; a < 3; ++a) {
+        if (gn && gn[a] < 1) { delete cx; return nullptr; }
+        cx->g.h[a] = 1.0 / (gn ? gn[a] : n[a]);
+        cx->ng[a] = ng[a];
+        cx->bc[a][0] = kinds[2 * a];
+        cx->bc[a][1] = kinds[2 * a + 1];
+    }
+    cx->gam = gamma;
+    cx->cfl = cfl;
+    cx->s.resize(cx->g.N);
+    return cx;
+}
+
 // Scheme switches of the paper; call before oracle_set_primitives.  With uct = 0 the three
 // "face" arrays of set/get_primitives are the CELL-CENTRED B.
 int oracle_set_scheme(void *h, int uct, int ho) {
@@ -689,6 +797,11 @@ int oracle_set_primitives(void *h, const double *rho, const double *vx, const do
     const Grid &g = cx->g;
     const double *bf[3] = {bxf, byf, bzf};
     for (int d = 0; d < 3; ++d) cx->s.Bf[d].assign(bf[d], bf[d] + g.N);
+    {   // bounded grids: the ghost layers of B come from the interior before INT reads them
+        Field dummy[5];
+        for (auto &f : dummy) f.assign(g.N, 0.0);
+        fill_ghosts(*cx, dummy, cx->s.Bf);
+    }
     Field Bc[3];
     if (cx->uct) centre_b(g, cx->s.Bf, Bc, cx->ho);
     else for (int d = 0; d < 3; ++d) Bc[d] = cx->s.Bf[d];   // UCT=NO: the arrays given are cell-centred
@@ -698,6 +811,7 @@ int oracle_set_primitives(void *h, const double *rho, const double *vx, const do
         prim2cons(cx->gam, q, u);
         for (int v = 0; v < 5; ++v) cx->s.U[v][c] = u[v];
     }
+    fill_ghosts(*cx, cx->s.U, cx->s.Bf);
     cx->t = 0.0; cx->dt_last = 0.0; cx->amax = 0.0; cx->steps = 0;
     cx->c2p = Stats(); cx->c2p_fail_total = 0;
     cx->has_state = true;
