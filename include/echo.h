@@ -108,7 +108,8 @@ int echo_faces_from_potential(echo_ctx *ctx, const double *ax, const double *ay,
  * reaches t_end: the last dt is clipped to t_end - t on the device and later steps are no-ops
  * (pass +inf to disable).  The time step is formed on the device from the stage-1 characteristic
  * speeds of the same step (S9).  No host synchronisation.  ECHO_EINVAL on a block
- * handle with halos (echo_create_block): those are stepped stage by stage by their owner. */
+ * handle with halos (echo_create_block) that the caller has to refresh: those are stepped stage by stage
+ * by their owner (a block whose padded sides are all physical boundaries, echo_set_boundaries, is fine). */
 int echo_step(echo_ctx *ctx, int nsteps, double t_end);
 
 /* Host loop around echo_step: advances until t >= t_end (last dt clipped), max_steps steps were taken, or a
@@ -196,6 +197,28 @@ int echo_diagnostics(echo_ctx *ctx, double *out);
  * echo_set_primitives / echo_get_primitives work on the padded block as on a plain box. */
 echo_ctx *echo_create_block(int nx, int ny, int nz, double gamma, double cfl, int gnx, int gny, int gnz,
                             int halo_x, int halo_y, int halo_z);
+
+/* ---- physical boundaries ("next" row f4, first slice: non-periodic boundaries in flat space) -----------------------
+ * Host only, before echo_set_primitives, on a handle made by echo_create_block with halo_d = 8 on the bounded axes
+ * (the paper's code keeps ghost cells that are filled before every stencil loop; here they are
+ * filled once per RK stage, which the 8 layers allow).  kinds (HOST, 6 ints) = {x_lo, x_hi, y_lo, y_hi, z_lo, z_hi}:
+ *   0  none: the axis is periodic (halo 0) or that halo is refreshed by the caller from a neighbouring block;
+ *   1  reflecting wall: ghost layers = mirror image of the interior with the parity of each field under the reflection
+ *      (scalars even, the momentum normal to the wall odd; B is axial: normal component even, tangential ones odd);
+ *   2  outflow: zero gradient (ghost layers = the nearest interior value).
+ * The wall lies on the face between the last ghost layer and the first interior cell: entry lo-1 (resp. hi-1) of the
+ * face array of the normal B is the wall face; it is evolved by the scheme and must be given in echo_set_primitives
+ * (all other ghost entries passed in are ignored and overwritten).  a_max, the con2prim failure count, the sums and the
+ * maximum of div B of echo_diagnostics look at the interior only.  A handle whose every padded side has a kind != 0 is
+ * advanced by echo_step / echo_run_until like a plain box (the ghost fill runs inside the step, after every stage).
+ * ECHO_EINVAL: bad kind, fewer than 8 ghost layers on that side, uct = 0.  ECHO_ESTATE once a state exists. */
+int echo_set_boundaries(echo_ctx *ctx, const int *kinds);
+
+/* The ghost fill itself, for callers that drive a block stage by stage (a block at the edge of a decomposed bounded
+ * domain: physical boundary on one side, neighbour on the other): fills the ghost layers of the 8 given workspace
+ * fields (HOST array; slots 0-4 are treated as D, S_x, S_y, S_z, U - or their rhs -, slots 5-7 as B_x, B_y, B_z; -1 =
+ * skip) on every side that has a boundary kind, axes in the order x, y, z.  No synchronisation. */
+int echo_fill_boundaries(echo_ctx *ctx, const int *fields);
 
 /* Host only.  Byte offset, inside the workspace given to echo_bind, of field `field` (0..43; 0-7 the state U^n =
  * D, Sx, Sy, Sz, U, Bx, By, Bz; 8-15 the stage state); each field is nx*ny*nz doubles. */

@@ -41,6 +41,8 @@ SIGNATURES = {
     "echo_div_b": (_int, [_vp, _vp, C.POINTER(_dbl)]),
     "echo_diagnostics": (_int, [_vp, C.POINTER(_dbl)]),
     "echo_create_block": (_vp, [_int, _int, _int, _dbl, _dbl, _int, _int, _int, _int, _int, _int]),
+    "echo_set_boundaries": (_int, [_vp, C.POINTER(_int)]),
+    "echo_fill_boundaries": (_int, [_vp, C.POINTER(_int)]),
     "echo_field_offset": (_sz, [_vp, _int]),
     "echo_ctrl_offset": (_sz, [_int]),
     "echo_stage_sweeps": (_int, [_vp, _int, _dbl]),
@@ -109,8 +111,10 @@ class EchoError(RuntimeError):
 class Echo:
     """One periodic unit box on the current CUDA device.  Tensors are torch.float64, shape (nz, ny, nx)."""
 
-    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True, uct=True, rec=5, rk=3):
+    def __init__(self, nx, ny, nz, gamma, cfl, device=None, block=None, ho=True, uct=True, rec=5, rk=3, boundaries=None):
         """block = (gnx, gny, gnz, halo_x, halo_y, halo_z): a domain-decomposition block (echo_create_block).
+        boundaries = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi), 0 none / 1 reflecting / 2 outflow (echo_set_boundaries): needs a
+        block with halo 8 on the bounded axes; nx, ny, nz are then the PADDED sizes.
         ho / uct: the paper's scheme switches (echo_set_scheme); with uct=False the three "face" arrays of
         set_primitives / get_primitives are the cell-centred B."""
         torch = _torch()
@@ -129,6 +133,8 @@ class Echo:
             self._check(self.L.echo_set_scheme(self.h, int(bool(uct)), int(bool(ho))))
         if (rec, rk) != (5, 3):     # echo_set_order: 2 / 2 = limited linear REC + SSP-RK2
             self._check(self.L.echo_set_order(self.h, int(rec), int(rk)))
+        if boundaries is not None:
+            self._check(self.L.echo_set_boundaries(self.h, (_int * 6)(*[int(k) for k in boundaries])))
         nbytes = self.L.echo_workspace_bytes(self.h)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # owned by the caller side
         # the stream of the workspace's device: the library runs every kernel of this handle there (echo_bind)
@@ -242,6 +248,9 @@ class Echo:
         self._check(self.L.echo_get_tiling(self.h, out))
         names = ["cx_flux", "cy_flux", "cz_flux", "cz_prim", "cz_uct", "cz_bupd", "tile_x", "tile_y"]
         return dict(zip(names, list(out)))
+
+    def fill_boundaries(self, fields):
+        self._check(self.L.echo_fill_boundaries(self.h, (_int * 8)(*[int(f) for f in fields])))
 
     def stage_halo_fields(self, stage):
         """The 8 workspace fields whose halos the next half needs after stage `stage` (5 cell fields, 3 face fields)."""

@@ -28,6 +28,7 @@ struct echo_ctx {
     bool bound = false, has_state = false;
     int rk = 3;              // SSP-RK3 or SSP-RK2 (echo_set_order)
     bool block = false;      // echo_create_block: explicit spacing, halos refreshed by the caller between stages
+    int bc[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // physical boundary per (axis, side) of a padded block: 0 none, 1 reflecting, 2 outflow
     bool gate_active = false;   // inside echo_step / echo_stage_*: con2prim failures count only while ctrl->active
     // one full step captured as a CUDA graph (echo_step replays it)
     cudaStream_t cap_stream = nullptr;    // capture target (the legacy default stream cannot be captured)
@@ -409,6 +410,34 @@ int launch_update(echo_ctx *ctx, const Stage &st, int cur_which, int out_which, 
     return ECHO_OK;
 }
 
+// ghost fill of the 8 given workspace fields (slots as in stage_halo_fields; -1 skipped) on every bounded side, axes in
+// the order x, y, z (row f4)
+int fill_boundaries(echo_ctx *ctx, const int *fields) {
+    const Grid &g = ctx->g;
+    HaloFields hf;
+    for (int v = 0; v < 8; ++v) hf.f[v] = fields[v] < 0 ? nullptr : ctx->field[fields[v]];
+    for (int a = 0; a < 3; ++a)
+        for (int side = 0; side < 2; ++side) {
+            const int kind = ctx->bc[a][side];
+            if (!kind) continue;
+            const int h = side == 0 ? g.lo[a] : g.n[a] - g.hi[a];
+            const long long per_field = (long long)h * (g.N / g.n[a]);
+            const int blocks = (int)std::min<long long>((per_field + 255) / 256, 148LL * 16);
+            if (kind == 1) KL(KC_OTHER, "k_fill_ghost", k_fill_ghost<1><<<dim3(blocks, 8), 256, 0, ctx->stream>>>(g, hf, a, side, per_field));
+            else KL(KC_OTHER, "k_fill_ghost", k_fill_ghost<2><<<dim3(blocks, 8), 256, 0, ctx->stream>>>(g, hf, a, side, per_field));
+        }
+    return ECHO_OK;
+}
+// true if no side of the padded block is left to the caller to refresh (plain periodic boxes included)
+bool self_contained(const echo_ctx *ctx) {
+    const Grid &g = ctx->g;
+    for (int a = 0; a < 3; ++a) {
+        if (g.lo[a] > 0 && !ctx->bc[a][0]) return false;
+        if (g.hi[a] < g.n[a] && !ctx->bc[a][1]) return false;
+    }
+    return true;
+}
+
 // Every launching call runs on the device of the bound workspace, whatever the calling thread's current device is,
 // and leaves the caller's current device as it found it.
 struct DevGuard {
@@ -513,10 +542,13 @@ int echo_set_primitives(echo_ctx *ctx, const double *rho, const double *vx, cons
     for (int d = 0; d < 3; ++d)
         if (bf[d] != ctx->field[F_BF + d])
             CU(cudaMemcpyAsync(ctx->field[F_BF + d], bf[d], sizeof(double) * g.N, cudaMemcpyDeviceToDevice, ctx->stream));
+    const int fB[8] = {-1, -1, -1, -1, -1, F_BF, F_BF + 1, F_BF + 2}, fU[8] = {F_U, F_U + 1, F_U + 2, F_U + 3, F_U + 4, -1, -1, -1};
+    if (ctx->block && (rc = fill_boundaries(ctx, fB))) return rc;   // bounded block: ghost faces before INT reads them
     KL(KC_OTHER, "k_init", k_init<<<cell_grid(g), cell_block(), 0, ctx->stream>>>(g, rho, vx, vy, vz, p, ctx->field[F_BF], ctx->field[F_BF + 1],
                                                            ctx->field[F_BF + 2], ctx->field[F_U], ctx->field[F_U + 1],
                                                            ctx->field[F_U + 2], ctx->field[F_U + 3], ctx->field[F_U + 4],
                                                            ctx->gg));
+    if (ctx->block && (rc = fill_boundaries(ctx, fU))) return rc;   // ... and the ghost cells of the conserved fields
     // the stage buffers are read (never trusted) by the passes of a step enqueued past t_end: give them defined contents
     CU(cudaMemsetAsync(ctx->field[F_U1], 0, sizeof(double) * (size_t)ctx->npad * 8, ctx->stream));
     Ctrl h;
@@ -625,6 +657,11 @@ static int enqueue_step(echo_ctx *ctx) {
     for (int stage = 1; stage <= ctx->rk; ++stage) {
         if ((rc = stage_sweeps_impl(ctx, stage))) return rc;
         if ((rc = stage_finish_impl(ctx, stage))) return rc;
+        if (ctx->block) {   // a bounded block: refill the ghost layers of what the next half reads (row f4)
+            int f[8];
+            stage_halo_fields(ctx, stage, f);
+            if ((rc = fill_boundaries(ctx, f))) return rc;
+        }
     }
     return ECHO_OK;
 }
@@ -666,8 +703,11 @@ int echo_step(echo_ctx *ctx, int nsteps, double t_end) {
     if (rc) return rc;
     DevGuard dev_guard_(ctx);
     if (nsteps < 0 || std::isnan(t_end)) return fail(ctx, ECHO_EINVAL, "nsteps < 0 or t_end is NaN");
-    if (ctx->block && (ctx->g.lo[0] > 0 || ctx->g.lo[1] > 0 || ctx->g.lo[2] > 0))
-        return fail(ctx, ECHO_EINVAL, "a block with halos is stepped stage by stage (echo_stage_sweeps / echo_stage_finish) by its owner");
+    if (ctx->block && !self_contained(ctx))
+        return fail(ctx, ECHO_EINVAL, "a block with halos is stepped stage by stage (echo_stage_sweeps / echo_stage_finish) by its owner, "
+                                      "unless every padded side has a physical boundary (echo_set_boundaries)");
+    if (ctx->block && !ctx->g.uct && (ctx->g.lo[0] || ctx->g.lo[1] || ctx->g.lo[2]))
+        return fail(ctx, ECHO_EINVAL, "padded blocks are built for UCT=YES only");
     GateScope gate_scope_(ctx);
     if (nsteps == 0) return ECHO_OK;
     KL(KC_CTRL, "k_set_t_end", k_set_t_end<<<1, 1, 0, ctx->stream>>>(ctx->ctrl, t_end));
@@ -690,7 +730,7 @@ int echo_run_until(echo_ctx *ctx, double t_end, long max_steps, long *steps_take
     if (rc) return rc;
     DevGuard dev_guard_(ctx);
     if (std::isnan(t_end) || max_steps < 0) return fail(ctx, ECHO_EINVAL, "t_end is NaN or max_steps < 0");
-    if (ctx->block) return fail(ctx, ECHO_EINVAL, "block handles are stepped stage by stage by their owner");
+    if (ctx->block && !self_contained(ctx)) return fail(ctx, ECHO_EINVAL, "block handles are stepped stage by stage by their owner");
     Ctrl h;
     CU(cudaMemcpyAsync(&h, ctx->ctrl, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -864,7 +904,7 @@ int echo_diagnostics(echo_ctx *ctx, double *out) {
     for (int m = 0; m < ECHO_NDIAG; ++m) out[m] = 0.0;
     double *f = ctx->field[F_U];
     const long long np = ctx->npad;
-    KL(KC_OTHER, "k_sums", k_sums<<<NPART, 256, 0, ctx->stream>>>(g.N, f, f + np, f + 2 * np, f + 3 * np, f + 4 * np, f + 5 * np, f + 6 * np,
+    KL(KC_OTHER, "k_sums", k_sums<<<NPART, 256, 0, ctx->stream>>>(g, f, f + np, f + 2 * np, f + 3 * np, f + 4 * np, f + 5 * np, f + 6 * np,
                                            f + 7 * np, ctx->part));
     Stage st = make_stage(ctx, 0);
     KL(KC_CTRL, "k_c2p_stats_reset", k_c2p_stats_reset<<<1, 1, 0, ctx->stream>>>(ctx->ctrl));
@@ -976,6 +1016,33 @@ int echo_stage_finish(echo_ctx *ctx, int stage) {
     if (stage < 1 || stage > ctx->rk) return fail(ctx, ECHO_EINVAL, "stage must be 1 .. number of RK stages");
     GateScope gate_scope_(ctx);
     return stage_finish_impl(ctx, stage);
+}
+
+int echo_set_boundaries(echo_ctx *ctx, const int *kinds) {
+    if (!ctx) return ECHO_EINVAL;
+    if (!kinds) return fail(ctx, ECHO_EINVAL, "null argument");
+    if (ctx->has_state) return fail(ctx, ECHO_ESTATE, "echo_set_boundaries must precede echo_set_primitives");
+    const Grid &g = ctx->g;
+    for (int a = 0; a < 3; ++a)
+        for (int side = 0; side < 2; ++side) {
+            const int k = kinds[2 * a + side], h = side == 0 ? g.lo[a] : g.n[a] - g.hi[a];
+            if (k < 0 || k > 2) return fail(ctx, ECHO_EINVAL, "boundary kind must be 0 (none), 1 (reflecting) or 2 (outflow)");
+            if (k && h < 8) return fail(ctx, ECHO_EINVAL, "a physical boundary needs 8 ghost layers on that axis (echo_create_block with halo 8)");
+            if (k && !g.uct) return fail(ctx, ECHO_EINVAL, "physical boundaries are built for UCT=YES only");
+        }
+    for (int a = 0; a < 3; ++a) { ctx->bc[a][0] = kinds[2 * a]; ctx->bc[a][1] = kinds[2 * a + 1]; }
+    ctx->drop_graph();
+    return ECHO_OK;
+}
+
+int echo_fill_boundaries(echo_ctx *ctx, const int *fields) {
+    int rc = check_ready(ctx, false);
+    if (rc) return rc;
+    DevGuard dev_guard_(ctx);
+    if (!fields) return fail(ctx, ECHO_EINVAL, "null argument");
+    for (int v = 0; v < 8; ++v)
+        if (fields[v] < -1 || fields[v] >= NFIELD) return fail(ctx, ECHO_EINVAL, "field index out of range");
+    return fill_boundaries(ctx, fields);
 }
 
 int echo_stage_halo_fields(const echo_ctx *ctx, int stage, int *fields) {

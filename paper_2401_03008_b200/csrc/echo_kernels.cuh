@@ -320,7 +320,9 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_flux(Grid g, Stage st, int C, 
                     st.vb[D][1][o] = vb2;
                 }
                 const int cD = m0 + f - 3, cTT = t0 + b, cOO = (int)blockIdx.z;
-                const bool inner = cD >= g.lo[D] && cD < g.hi[D] && cTT >= g.lo[TD] && cTT < g.hi[TD] &&
+                // faces of the interior: entry c is the face on the + side of cell c, so along D the face lo-1 (the low
+                // wall of a bounded block, or the neighbour's last face of a decomposed one) belongs to it as well
+                const bool inner = cD >= g.lo[D] - (g.lo[D] > 0) && cD < g.hi[D] && cTT >= g.lo[TD] && cTT < g.hi[TD] &&
                                    cOO >= g.lo[OD] && cOO < g.hi[OD];
                 if (inner) amax = dmax(amax, dmax(ap, am));
             }
@@ -415,7 +417,10 @@ __global__ void __launch_bounds__(256) k_flux_flat(Grid g, Stage st, double gam,
         } else {
             hll_face_cc<D>(gam, gg, qL, qR, F, ap, am);
         }
-        const bool inner = i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2];
+        const int c3[3] = {i, j, k};
+        bool inner = true;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) inner = inner && c3[a] >= g.lo[a] - ((a == D && g.lo[a] > 0) ? 1 : 0) && c3[a] < g.hi[a];
         if (inner) amax = dmax(ap, am);
         if (MODE == 1) {
             const double dt = ctrl->dt;
@@ -540,7 +545,9 @@ __global__ void __launch_bounds__(256) k_divb(Grid g, const double *B0, const do
             v += g.rh[d] * der_diff_ho(g.ho, f[0], f[1], f[2], f[3], f[4], f[5]);
         }
         if (div) div[c] = v;
-        v = fabs(v);
+        // the maximum looks at the interior of a padded block only (its outflow ghost layers are not solenoidal)
+        const bool inner = i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2];
+        v = inner ? fabs(v) : 0.0;
     }
     __shared__ double sm[256];
     const int tid = threadIdx.y * blockDim.x + threadIdx.x;
@@ -578,19 +585,71 @@ __global__ void __launch_bounds__(256) k_halo_copy(Grid g, HaloFields hf, double
     }
 }
 
+// ------------------------------------------------------------------ physical boundaries (row f4, first slice)
+// Ghost fill of 8 fields (slots 0-4: the cell fields D, S_x, S_y, S_z, U or their rhs; slots 5-7: the face fields
+// B_x, B_y, B_z) on ONE side of ONE axis `a` of a padded block, ghost layers m = 0 .. h-1, over the full padded extent
+// of the other axes (edges and corners get the composition when the axes are filled in the order x, y, z):
+//   kind 1, reflecting wall: the mirror image with the parity of each field under the reflection (scalars even, the
+//           momentum normal to the wall odd; B axial: normal component even, tangential ones odd);
+//   kind 2, outflow: zero gradient, the nearest interior value.
+// Fields centred along a:  low ghost lo-1-m <- lo+m (lo),  high ghost hi+m <- hi-1-m (hi-1).  B_a is staggered along
+// a (entry c = face on the + side of cell c): the wall faces lo-1 and hi-1 are evolved by the scheme, ghost faces
+// lo-1-m <- lo-1+m (lo-1) and hi-1+m <- hi-1-m (hi-1) for m >= 1.  blockIdx.y = slot; a null field is skipped.
+template <int KIND>
+__global__ void __launch_bounds__(256) k_fill_ghost(Grid g, HaloFields hf, int a, int side, long long per_field) {
+    const int slot = blockIdx.y;
+    double *f = hf.f[slot];
+    if (!f) return;
+    const int lo = g.lo[a], hi = g.hi[a];
+    const int h = side == 0 ? lo : g.n[a] - hi;              // ghost layers on this side
+    int d[3] = {g.n[0], g.n[1], g.n[2]};
+    d[a] = h;
+    const bool normalB = slot == 5 + a;
+    const double sgn = (KIND == 1 && (slot == 1 + a || (slot >= 5 && !normalB))) ? -1.0 : 1.0;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < per_field; t += (long long)gridDim.x * blockDim.x) {
+        int c[3];
+        c[0] = (int)(t % d[0]);
+        c[1] = (int)((t / d[0]) % d[1]);
+        c[2] = (int)(t / ((long long)d[0] * d[1]));
+        const int m = c[a];                                   // ghost layer 0 .. h-1 (distance from the interior)
+        const int ghost = side == 0 ? lo - 1 - m : hi + m;
+        int src;
+        if (!normalB) {
+            src = KIND == 1 ? (side == 0 ? lo + m : hi - 1 - m) : (side == 0 ? lo : hi - 1);
+        } else {
+            const int mf = side == 0 ? m : m + 1;             // distance of this face from the wall face
+            if (mf == 0) continue;                            // the low wall face is evolved, not filled
+            src = KIND == 1 ? (side == 0 ? lo - 1 + mf : hi - 1 - mf) : (side == 0 ? lo - 1 : hi - 1);
+        }
+        c[a] = 0;
+        const long long base = c[0] + (long long)g.s[1] * c[1] + (long long)g.s[2] * c[2];
+        f[base + (long long)g.s[a] * ghost] = sgn * f[base + (long long)g.s[a] * src];
+    }
+}
+
 // ------------------------------------------------------------------ deterministic reductions
 // NPART contiguous chunks; each block sums its chunk with a fixed tree, the host adds the NPART
 // partials in extended precision.  rows 0..7: sums of the 8 evolved fields.
-__global__ void __launch_bounds__(256) k_sums(long long N, const double *f0, const double *f1, const double *f2,
+__global__ void __launch_bounds__(256) k_sums(Grid g, const double *f0, const double *f1, const double *f2,
                                               const double *f3, const double *f4, const double *f5,
                                               const double *f6, const double *f7, double *part) {
     const double *f[8] = {f0, f1, f2, f3, f4, f5, f6, f7};
+    const long long N = g.N;
     const long long chunk = (N + NPART - 1) / NPART;
     const long long lo = chunk * blockIdx.x, hi = min(N, lo + chunk);
+    // a padded block (domain decomposition, physical boundaries) sums its interior only
+    const bool padded = g.lo[0] > 0 || g.lo[1] > 0 || g.lo[2] > 0 || g.hi[0] < g.n[0] || g.hi[1] < g.n[1] || g.hi[2] < g.n[2];
     __shared__ double sm[256];
     for (int v = 0; v < 8; ++v) {
         double s = 0.0;
-        for (long long c = lo + threadIdx.x; c < hi; c += 256) s += f[v][c];
+        for (long long c = lo + threadIdx.x; c < hi; c += 256) {
+            bool in = true;
+            if (padded) {
+                const int i = (int)(c % g.n[0]), j = (int)((c / g.n[0]) % g.n[1]), k = (int)(c / ((long long)g.n[0] * g.n[1]));
+                in = i >= g.lo[0] && i < g.hi[0] && j >= g.lo[1] && j < g.hi[1] && k >= g.lo[2] && k < g.hi[2];
+            }
+            if (in) s += f[v][c];
+        }
         sm[threadIdx.x] = s;
         __syncthreads();
         for (int w = 128; w > 0; w >>= 1) {
