@@ -424,15 +424,8 @@ def run_gpu(args):
 
 
 def kernel_source_hash():
-    """sha256 over the CUDA sources the library is built from: ties an ncu capture to the kernels it measured."""
-    import hashlib
-    h = hashlib.sha256()
-    d = os.path.join(ROOT, "paper_2401_03008_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
-            h.update(f.encode())
-            h.update(open(os.path.join(d, f), "rb").read())
-    return h.hexdigest()
+    from paper_2401_03008_b200.ncu_summary import kernel_source_hash as h
+    return h()
 
 
 def measured_traffic(kernel_class, cells, args):
