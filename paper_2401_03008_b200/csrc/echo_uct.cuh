@@ -260,6 +260,29 @@ namespace echo {
 constexpr int BU_XE = UCT_XRW * UCT_TY;     // 21 x 8, x offsets -3 .. TX+1
 constexpr int BU_YE = UCT_TX * UCT_YRH;     // 16 x 13, y offsets -3 .. TY+1
 
+// curl (O8) + RK combination (O9) of the three face fields of ONE cell from its stencils: pz_x / py_x = E_z / E_y along
+// x, pz_y / px_y = E_z / E_x along y (stride S), wy / wx = E_y / E_x along z; bc / bb = current and base B of the cell.
+// Shared by k_bupd and k_bupd_flat so that the two stay bit-identical.
+__device__ __forceinline__ void bupd_cell(const Grid &g, const double *pz_x, const double *py_x, const double *pz_y,
+                                          const double *px_y, int S, const double wy[6], const double wx[6],
+                                          const double bc[3], const double bb[3], const Update &up, double dt, int o) {
+    const double dxEz = der_diff_ho(g.ho, pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
+    const double dxEy = der_diff_ho(g.ho, py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
+    const double dyEz = der_diff_ho(g.ho, pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
+    const double dyEx = der_diff_ho(g.ho, px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
+    const double dzEy = der_diff_ho(g.ho, wy[0], wy[1], wy[2], wy[3], wy[4], wy[5]);
+    const double dzEx = der_diff_ho(g.ho, wx[0], wx[1], wx[2], wx[3], wx[4], wx[5]);
+    double rb[3];
+    rb[0] = -(g.rh[1] * dyEz - g.rh[2] * dzEy);
+    rb[1] = -(g.rh[2] * dzEx - g.rh[0] * dxEz);
+    rb[2] = -(g.rh[0] * dxEy - g.rh[1] * dyEx);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double adv = bc[d] + dt * rb[d];
+        up.out[5 + d][o] = (up.c0 == 0.0) ? adv : up.c0 * bb[d] + up.c1 * adv;
+    }
+}
+
 __global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const double *E1, const double *E2, Update up,
                                                  const Ctrl *ctrl, int CZ) {
     __shared__ double sXE[2][2][BU_XE];    // fields: E_z, E_y (differenced along x)
@@ -333,23 +356,7 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd(Grid g, const double *E0, const
             const int ps = r & 1;
             const double *pz_x = &sXE[ps][0][ty * UCT_XRW + tx], *py_x = pz_x + BU_XE;     // E_z, E_y along x
             const double *pz_y = &sYE[ps][0][ty * UCT_TX + tx], *px_y = pz_y + BU_YE;      // E_z, E_x along y
-            constexpr int S = UCT_TX;
-            const double dxEz = der_diff_ho(g.ho, pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
-            const double dxEy = der_diff_ho(g.ho, py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
-            const double dyEz = der_diff_ho(g.ho, pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
-            const double dyEx = der_diff_ho(g.ho, px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
-            const double dzEy = der_diff_ho(g.ho, wy[0], wy[1], wy[2], wy[3], wy[4], wy[5]);
-            const double dzEx = der_diff_ho(g.ho, wx[0], wx[1], wx[2], wx[3], wx[4], wx[5]);
-            double rb[3];
-            rb[0] = -(g.rh[1] * dyEz - g.rh[2] * dzEy);
-            rb[1] = -(g.rh[2] * dzEx - g.rh[0] * dxEz);
-            rb[2] = -(g.rh[0] * dxEy - g.rh[1] * dyEx);
-            const int o = sz * k + ccol;
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const double adv = bc[d] + dt * rb[d];
-                up.out[5 + d][o] = (up.c0 == 0.0) ? adv : up.c0 * bb[d] + up.c1 * adv;
-            }
+            bupd_cell(g, pz_x, py_x, pz_y, px_y, UCT_TX, wy, wx, bc, bb, up, dt, sz * k + ccol);
         }
 #pragma unroll
         for (int m = 0; m < 5; ++m) { wy[m] = wy[m + 1]; wx[m] = wx[m + 1]; }
@@ -559,23 +566,9 @@ __global__ void __launch_bounds__(UCT_NT) k_bupd_flat(Grid g, const double *E0, 
             const int ps = r & 1;
             const double *pz_x = &sXE[ps][0][ty * UCT_XRW + tx], *py_x = pz_x + BU_XE;
             const double *pz_y = &sYE[ps][0][ty * UCT_TX + tx], *px_y = pz_y + BU_YE;
-            constexpr int S = UCT_TX;
-            const double dxEz = der_diff_ho(g.ho, pz_x[0], pz_x[1], pz_x[2], pz_x[3], pz_x[4], pz_x[5]);
-            const double dxEy = der_diff_ho(g.ho, py_x[0], py_x[1], py_x[2], py_x[3], py_x[4], py_x[5]);
-            const double dyEz = der_diff_ho(g.ho, pz_y[0], pz_y[S], pz_y[2 * S], pz_y[3 * S], pz_y[4 * S], pz_y[5 * S]);
-            const double dyEx = der_diff_ho(g.ho, px_y[0], px_y[S], px_y[2 * S], px_y[3 * S], px_y[4 * S], px_y[5 * S]);
-            const double dzEy = der_diff_ho(g.ho, ec[0], ec[0], ec[0], ec[0], ec[0], ec[0]);
-            const double dzEx = der_diff_ho(g.ho, ec[1], ec[1], ec[1], ec[1], ec[1], ec[1]);
-            double rb[3];
-            rb[0] = -(g.rh[1] * dyEz - g.rh[2] * dzEy);
-            rb[1] = -(g.rh[2] * dzEx - g.rh[0] * dxEz);
-            rb[2] = -(g.rh[0] * dxEy - g.rh[1] * dyEx);
-            const int o = cell(t);
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const double adv = bc[d] + dt * rb[d];
-                up.out[5 + d][o] = (up.c0 == 0.0) ? adv : up.c0 * bb[d] + up.c1 * adv;
-            }
+            const double wy[6] = {ec[0], ec[0], ec[0], ec[0], ec[0], ec[0]};      // the z-stencils of a one-plane grid:
+            const double wx[6] = {ec[1], ec[1], ec[1], ec[1], ec[1], ec[1]};      // six times the cell's own value
+            bupd_cell(g, pz_x, py_x, pz_y, px_y, UCT_TX, wy, wx, bc, bb, up, dt, cell(t));
         }
         ec[0] = nec[0]; ec[1] = nec[1];
 #pragma unroll
