@@ -94,12 +94,13 @@ def unpack_slabs(tensors, axis, side, buf, h=HALO):
             dst.copy_(buf[v * per:(v + 1) * per].view(dst.shape))
 
 
-def exchange_packed(decomp, rank, dist, bufs, pack, unpack, part=None):
+def exchange_packed(decomp, rank, dist, bufs, pack, unpack, part=None, group=None):
     """One halo refresh with packed messages: per decomposed axis (x, then y, then z, so that edges and corners
     arrive through the later axes) pack the two interior slabs, exchange them with the two neighbours (2 sends +
     2 receives instead of 4 per field), unpack into the two halos.  bufs[axis] = (send_lo, send_hi, recv_lo,
     recv_hi), persistent 1-D tensors; pack(axis, side, buf) / unpack(axis, side, buf) move the slabs; part(axis), if
-    given, is the slice of the buffers that is sent (the cell fields and the face fields of a stage travel separately)."""
+    given, is the slice of the buffers that is sent (the cell fields and the face fields of a stage travel separately);
+    group: the process group (communicator) to send on."""
     for axis in range(3):
         if decomp.p[axis] == 1:
             continue
@@ -110,8 +111,8 @@ def exchange_packed(decomp, rank, dist, bufs, pack, unpack, part=None):
         pack(axis, 1, send_hi)
         # order matters when lo == hi (two blocks along the axis): the peer's first message is its low slab, which
         # belongs in our HIGH halo
-        ops = [dist.P2POp(dist.isend, send_lo[sl], lo), dist.P2POp(dist.isend, send_hi[sl], hi),
-               dist.P2POp(dist.irecv, recv_hi[sl], hi), dist.P2POp(dist.irecv, recv_lo[sl], lo)]
+        ops = [dist.P2POp(dist.isend, send_lo[sl], lo, group), dist.P2POp(dist.isend, send_hi[sl], hi, group),
+               dist.P2POp(dist.irecv, recv_hi[sl], hi, group), dist.P2POp(dist.irecv, recv_lo[sl], lo, group)]
         for req in dist.batch_isend_irecv(ops):
             req.wait()          # NCCL: the current stream waits (no host block); gloo: the host waits
         unpack(axis, 0, recv_lo)
@@ -222,20 +223,24 @@ class RankBlock:
         self.bufs = [tuple(torch.empty(b.halo_doubles(ax), dtype=torch.float64, device=b.device) for _ in range(4))
                      if self.d.p[ax] > 1 else None for ax in range(3)]
         self.side = torch.cuda.Stream(device=b.device) if self.d.size > 1 else None
+        # the messages of the side stream travel on their own communicator: NCCL operations of ONE communicator must not
+        # run concurrently from two streams (the a_max all-reduce and the face messages use the default group)
+        self.side_group = dist.new_group() if self.d.size > 1 else None
 
     def set_primitives(self, w, keys=("rho", "vx", "vy", "vz", "p", "bxf", "byf", "bzf")):
         import torch
         self.block.set_primitives(*[torch.as_tensor(self.d.cut(self.rank, w[k]), device=self.block.device)
                                     for k in keys])
 
-    def _exchange(self, fields, part, stream):
+    def _exchange(self, fields, part, stream, group=None):
         b = self.block
         f = _masked(fields, part)
         sp = stream.cuda_stream if stream is not None else None
         exchange_packed(self.d, self.rank, self.dist, self.bufs,
                         lambda ax, side, buf: b.halo_pack(f, ax, side, buf, sp),
                         lambda ax, side, buf: b.halo_unpack(f, ax, side, buf, sp),
-                        part=lambda ax: slice(part.start * (b.halo_doubles(ax) // 8), part.stop * (b.halo_doubles(ax) // 8)))
+                        part=lambda ax: slice(part.start * (b.halo_doubles(ax) // 8), part.stop * (b.halo_doubles(ax) // 8)),
+                        group=group)
 
     def step(self, nsteps, t_end=math.inf):
         import torch
@@ -248,7 +253,7 @@ class RankBlock:
                 if self.side is not None:                    # cell fields: exchanged under the UCT kernels
                     self.side.wait_stream(main)
                     with torch.cuda.stream(self.side):
-                        self._exchange(fields, CELLS, self.side)
+                        self._exchange(fields, CELLS, self.side, self.side_group)
                 if stage == 1:
                     dist.all_reduce(b.ctrl_word(0), op=dist.ReduceOp.MAX)
                 b.stage_finish(stage)

@@ -43,11 +43,13 @@ def per(axis):
 bufs = [tuple(torch.full((8 * per(ax),), -7.0, dtype=torch.float64) for _ in range(4)) if d.p[ax] > 1 else None for ax in range(3)]
 cells = [ts[0], ts[1], ts[0], ts[1], ts[0], None, None, None]
 faces = [None] * 5 + [ts[1], ts[0], ts[1]]
+side_group = dist.new_group()            # as RankBlock: the cell part travels on its own communicator
 for tensors, part in ((cells, blocks.CELLS), (faces, blocks.FACES)):
     blocks.exchange_packed(d, rank, dist, bufs,
                            lambda ax, side, buf: blocks.pack_slabs(tensors, ax, side, buf),
                            lambda ax, side, buf: blocks.unpack_slabs(tensors, ax, side, buf),
-                           part=lambda ax: slice(part.start * per(ax), part.stop * per(ax)))
+                           part=lambda ax: slice(part.start * per(ax), part.stop * per(ax)),
+                           group=side_group if part is blocks.CELLS else None)
     if part is blocks.CELLS:      # after the first part every halo is already restored (both tensors travelled)
         ok_first = all(np.array_equal(t.numpy(), d.cut(rank, a)) for t, a in zip(ts, glob))
 ok = ok_first and all(np.array_equal(t.numpy(), d.cut(rank, a)) for t, a in zip(ts, glob))
