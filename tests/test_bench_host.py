@@ -64,3 +64,34 @@ def test_clock_sampler_and_bookkeeping():
     # per-stage doubles of the kernels as built sum to the documented 2784 B per cell-update
     assert abs(bench.BYTES_PER_CELL_UPDATE - 2784.0) < 1e-9
     assert 8300 < bench.FLOP_PER_CELL_UPDATE < 8700
+
+
+def test_traffic_comes_from_the_committed_capture_or_is_null(tmp_path, monkeypatch):
+    """roofline.traffic is read from profiles/r2_traffic.json and only trusted when the capture ran on the CUDA sources
+    of this tree (sha256 stamp), on the same scheme and workload; otherwise null with the reason."""
+    import argparse
+    import bench
+    from paper_2401_03008_b200 import ncu_summary as ns
+    assert ns.kernel_class("void k_flux<1, 128, 0, 1, 1, 5>(Grid, Stage, int, double, double, Ctrl *, int, FluxUpd)") == "k_flux_y"
+    assert ns.kernel_class("void k_uct3<0, 8>(Grid, Stage, int, UctMaps)") == "k_uct"
+    assert ns.kernel_class("k_bupd(Grid, const double *, const double *, const double *, Update, const Ctrl *, int)") == "k_update"
+    assert ns.kernel_class("void k_prim_march<1>(Grid, Stage, double, Ctrl *, PrimUpd, int, const int *)") == "k_prim"
+    assert ns.kernel_class("k_set_dt(Ctrl *, double)") is None
+    h = ns.kernel_source_hash()
+    assert len(h) == 64 and h == bench.kernel_source_hash()
+    args = argparse.Namespace(scheme="uct-ho", workload="cpa")
+    (tmp_path / "profiles").mkdir()
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    t, why = bench.measured_traffic("k_uct", 1000, args)
+    assert t is None and "no ncu capture" in why
+    cap = {"source_sha256": h, "scheme": "uct-ho", "n": 256, "report": "x.ncu-rep", "md": "profiles/x.md",
+           "kernels": {"k_uct": {"kernel": "k_uct3", "dram_bytes_per_cell": 164.0}}}
+    (tmp_path / "profiles" / "r2_traffic.json").write_text(json.dumps(cap))
+    t, why = bench.measured_traffic("k_uct", 1000, args)
+    assert t == 164.0 * 1000 and "dram__bytes" in why
+    assert bench.measured_traffic("k_prim", 1000, args)[0] is None
+    assert bench.measured_traffic("k_uct", 1000, argparse.Namespace(scheme="cc-lo", workload="cpa"))[0] is None
+    cap["source_sha256"] = "0" * 64                                   # captured on other kernels: not trusted
+    (tmp_path / "profiles" / "r2_traffic.json").write_text(json.dumps(cap))
+    t, why = bench.measured_traffic("k_uct", 1000, args)
+    assert t is None and "other kernel sources" in why
