@@ -239,10 +239,12 @@ def test_x_aligned_wave_dimensional_reduction(torch, eb):
         assert np.array_equal(a, np.broadcast_to(b, a.shape)), k
 
 
-def test_translation_covariance_bitwise(torch, eb, ob):
+@pytest.mark.parametrize("shape", [(40, 24, 20), (80, 40, 12)])
+def test_translation_covariance_bitwise(torch, eb, ob, shape):
     """P7(ii) on the GPU path: rolling every input by (3,5,7) cells rolls every output identically,
-    bit for bit — catches any periodic-wrap or tile-seam error."""
-    shape = (40, 24, 20)
+    bit for bit — catches any periodic-wrap or tile-seam error.  On 80 x 40 x 12 the UCT kernel moves the tiles inside
+    the grid by TMA and those on the periodic seams by cp.async: the roll carries cells from one kind of tile to the
+    other, so the two copy paths must deliver identical tiles."""
     w = turb_inputs(torch, eb, ob, None, shape=shape)
     roll = lambda a: np.roll(a, (7, 5, 3), axis=(0, 1, 2))
     e0 = eb.Echo(*shape, G, 0.3)
