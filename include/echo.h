@@ -172,6 +172,31 @@ int echo_prim2cons(double gamma, long n, const double *rho, const double *vx, co
  * may be NULL.  Synchronises. */
 int echo_div_b(echo_ctx *ctx, double *div_field, double *max_abs_host);
 
+/* The same divergence (S10) for callers that may not allocate: no handle, no workspace, no cudaMalloc,
+ * cudaFree or allocating library routine, no synchronisation -- two kernel launches on cuda_stream, legal under
+ * stream capture once echo_div_b_static_setup has run on the device.  Periodic unit box of nx*ny*nz cells (h_d =
+ * 1/n_d, x fastest), ho as in echo_set_scheme; bx/by/bz_face: device, N doubles each, entry c = face on the + side
+ * of cell c (the layout of echo_set_primitives).  Outputs (device, written asynchronously on cuda_stream):
+ * div_field (N doubles) may be NULL; max_abs_dev (ONE double, the maximum of |div B|) may be NULL; not both.
+ * Scratch: one partial maximum per tile of 64 x 4 x 1 cells in a static device array of
+ * ECHO_DIV_B_STATIC_MAX_TILES doubles (512 KiB, held by every GPU that loads the library until exit), so
+ *     ceil(nx/64) * ceil(ny/4) * nz <= ECHO_DIV_B_STATIC_MAX_TILES      (256^3 fits exactly);
+ * a larger grid returns ECHO_EINVAL before anything is launched, with the sizes in echo_div_b_static_error().
+ * The array is shared by every call on a device and keeps the last call's contents; each call overwrites every
+ * slot it reads, so nothing needs clearing, but two calls that can overlap on the GPU (different streams, no
+ * ordering between them) race on it: serialise them.  Results equal echo_div_b's (same arithmetic per cell).
+ * Errors: ECHO_EINVAL (sizes, null pointers), ECHO_ECUDA (symbol lookup or launch failed). */
+#define ECHO_DIV_B_STATIC_MAX_TILES 65536
+int echo_div_b_static(int nx, int ny, int nz, int ho, const double *bx_face, const double *by_face,
+                      const double *bz_face, double *div_field, double *max_abs_dev, void *cuda_stream);
+
+/* Host only.  Looks up the device address of the static scratch for the CURRENT device (once per device; later
+ * calls return at once).  echo_div_b_static calls it itself; call it before stream capture begins. */
+int echo_div_b_static_setup(void);
+
+/* Host only.  Message of the last failed echo_div_b_static[_setup] call of this thread ("" if none). */
+const char *echo_div_b_static_error(void);
+
 /* out (HOST, ECHO_NDIAG doubles) = {t, dt_last, steps, amax, sum D, sum Sx, sum Sy, sum Sz, sum U
  * (each x cell volume), sum Bx, sum By, sum Bz over faces (x volume), max|div_HO B|, max W,
  * min rho, min p, con2prim max iterations, con2prim mean iterations (both of the pass run by this

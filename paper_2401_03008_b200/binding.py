@@ -39,6 +39,9 @@ SIGNATURES = {
     "echo_con2prim": (_int, [_dbl, _long] + [_vp] * 13 + [_vp, _vp]),
     "echo_prim2cons": (_int, [_dbl, _long] + [_vp] * 13 + [_vp]),
     "echo_div_b": (_int, [_vp, _vp, C.POINTER(_dbl)]),
+    "echo_div_b_static": (_int, [_int, _int, _int, _int, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "echo_div_b_static_setup": (_int, []),
+    "echo_div_b_static_error": (C.c_char_p, []),
     "echo_diagnostics": (_int, [_vp, C.POINTER(_dbl)]),
     "echo_create_block": (_vp, [_int, _int, _int, _dbl, _dbl, _int, _int, _int, _int, _int, _int]),
     "echo_set_boundaries": (_int, [_vp, C.POINTER(_int)]),
@@ -57,6 +60,7 @@ SIGNATURES = {
     "echo_get_timing": (_int, [_vp, C.POINTER(_dbl), C.POINTER(_long)]),
     "echo_fp64_peak": (_int, [_int, C.POINTER(_dbl), _vp]),
 }
+ECHO_DIV_B_STATIC_MAX_TILES = 65536
 ECHO_NKCLASS = 8
 KCLASS_NAMES = ["k_prim", "k_flux_x", "k_flux_y", "k_flux_z", "k_uct", "k_update", "control", "other"]
 
@@ -294,6 +298,22 @@ def fp64_peak(reps=20):
     if rc:
         raise EchoError(rc, "echo_fp64_peak")
     return out[0], out[1]
+
+
+def div_b_static(bx_face, by_face, bz_face, ho=1, div_field=None, max_abs=None):
+    """echo_div_b_static: div B of (nz, ny, nx) FP64 CUDA face arrays on the periodic unit box into the CALLER's
+    outputs -- div_field (same shape) and/or max_abs (one double on the device), written asynchronously on the current
+    stream.  Allocates nothing; grids beyond ECHO_DIV_B_STATIC_MAX_TILES tiles of 64 x 4 x 1 cells raise EchoError."""
+    torch = _torch()
+    nz, ny, nx = bx_face.shape
+    n = nx * ny * nz
+    L = lib()
+    with torch.cuda.device(bx_face.device):      # the scratch address is the current device's
+        rc = L.echo_div_b_static(nx, ny, nz, int(ho), _dev(bx_face, n), _dev(by_face, n), _dev(bz_face, n),
+                                 _dev(div_field, n) if div_field is not None else None,
+                                 _dev(max_abs, 1) if max_abs is not None else None, _stream(bx_face.device))
+    if rc:
+        raise EchoError(rc, L.echo_div_b_static_error().decode())
 
 
 def _host_ptr(a, n):

@@ -1183,3 +1183,138 @@ int echo_fp64_peak(int reps, double *tflops_host, void *cuda_stream) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ allocation-free div B (echo_div_b_static)
+// For callers that may not allocate (code under stream capture, tight serving loops): the high-order div B of
+// echo_div_b, stateless, with its scratch -- one partial maximum per 64 x 4 x 1 tile of cells -- in a file-scope device
+// array instead of a workspace the caller would have had to cudaMalloc.  Every GPU that loads the library holds the
+// ECHO_DIV_B_STATIC_MAX_TILES * 8 bytes (512 KiB) until the process exits.  In HOST code the name g_divb_static is only
+// a stand-in for the symbol, not a device address: the address is looked up once per device with that device current
+// (cudaGetSymbolAddress) and handed to the kernels as a plain pointer.
+static __device__ __align__(256) double g_divb_static[ECHO_DIV_B_STATIC_MAX_TILES];
+
+namespace {
+
+constexpr int DIVB_TX = 64, DIVB_TY = 4;       // the tile of cell_block()
+constexpr int DIVB_MAX_DEVICES = 64;
+double *g_divb_static_ptr[DIVB_MAX_DEVICES] = {nullptr};   // device address of g_divb_static, per device ordinal
+thread_local char g_divb_static_err[192] = "";
+
+int divb_static_fail(int rc, const char *msg) {
+    std::snprintf(g_divb_static_err, sizeof(g_divb_static_err), "%s", msg);
+    return rc;
+}
+
+// Variant of k_divb: same stencil and the same order of operations per cell; the block's maximum of |div B| goes to
+// partial[linear tile index] (every slot the finishing kernel reads is written by this launch, so nothing has to be
+// cleared between calls).  1-D grid of tiles: blockIdx.x = tx + ntx * (ty + nty * k).
+__global__ void __launch_bounds__(256) k_divb_static(Grid g, int ntx, int nty, const double *B0, const double *B1,
+                                                     const double *B2, double *div, double *partial) {
+    const int tile = blockIdx.x;
+    const int i = (tile % ntx) * DIVB_TX + threadIdx.x;
+    const int j = ((tile / ntx) % nty) * DIVB_TY + threadIdx.y;
+    const int k = tile / (ntx * nty);
+    double v = 0.0;
+    if (i < g.n[0] && j < g.n[1]) {
+        const int c3[3] = {i, j, k};
+        const int c = i + g.s[1] * j + g.s[2] * k;
+        const double *B[3] = {B0, B1, B2};
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const int base = c - g.s[d] * c3[d];
+            double f[6];
+#pragma unroll
+            for (int m = 0; m < 6; ++m) f[m] = __ldg(B[d] + (base + g.s[d] * wrapi(c3[d] + m - 3, g.n[d])));
+            v += g.rh[d] * der_diff_ho(g.ho, f[0], f[1], f[2], f[3], f[4], f[5]);
+        }
+        if (div) div[c] = v;
+        v = fabs(v);
+    }
+    __shared__ double sm[256];
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    sm[tid] = v;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (tid < s) sm[tid] = fmax(sm[tid], sm[tid + s]);
+        __syncthreads();
+    }
+    if (tid == 0) partial[tile] = sm[0];
+}
+
+// one block: maximum of the first ntiles partials -> *out
+__global__ void __launch_bounds__(256) k_divb_static_finish(int ntiles, const double *partial, double *out) {
+    double v = 0.0;
+    for (int t = threadIdx.x; t < ntiles; t += 256) v = fmax(v, partial[t]);
+    __shared__ double sm[256];
+    sm[threadIdx.x] = v;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sm[threadIdx.x] = fmax(sm[threadIdx.x], sm[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sm[0];
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *echo_div_b_static_error(void) { return g_divb_static_err; }
+
+int echo_div_b_static_setup(void) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return divb_static_fail(ECHO_ECUDA, "echo_div_b_static: no current CUDA device");
+    if (dev < 0 || dev >= DIVB_MAX_DEVICES) return divb_static_fail(ECHO_EINVAL, "echo_div_b_static: device ordinal beyond 63");
+    if (g_divb_static_ptr[dev]) return ECHO_OK;
+    double *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_divb_static);
+    if (e != cudaSuccess || !ptr) {
+        char msg[160];
+        std::snprintf(msg, sizeof(msg), "echo_div_b_static: cudaGetSymbolAddress failed: %s", cudaGetErrorString(e));
+        return divb_static_fail(ECHO_ECUDA, msg);
+    }
+    g_divb_static_ptr[dev] = ptr;     // idempotent: two threads racing here store the same address
+    return ECHO_OK;
+}
+
+int echo_div_b_static(int nx, int ny, int nz, int ho, const double *bx_face, const double *by_face,
+                      const double *bz_face, double *div_field, double *max_abs_dev, void *cuda_stream) {
+    if (nx < 1 || ny < 1 || nz < 1) return divb_static_fail(ECHO_EINVAL, "echo_div_b_static: nx, ny, nz must be >= 1");
+    if (!bx_face || !by_face || !bz_face) return divb_static_fail(ECHO_EINVAL, "echo_div_b_static: null face array");
+    if (!div_field && !max_abs_dev) return divb_static_fail(ECHO_EINVAL, "echo_div_b_static: both outputs are null");
+    const long long ntx = (nx + DIVB_TX - 1) / DIVB_TX, nty = (ny + DIVB_TY - 1) / DIVB_TY;
+    const long long ntiles = ntx * nty * (long long)nz;
+    if (ntiles > ECHO_DIV_B_STATIC_MAX_TILES) {
+        char msg[192];
+        std::snprintf(msg, sizeof(msg),
+                      "echo_div_b_static: grid %d x %d x %d needs %lld tiles of 64 x 4 x 1 cells, the static scratch holds %d "
+                      "(e.g. 256^3); use echo_div_b",
+                      nx, ny, nz, ntiles, ECHO_DIV_B_STATIC_MAX_TILES);
+        return divb_static_fail(ECHO_EINVAL, msg);
+    }
+    int rc = echo_div_b_static_setup();
+    if (rc) return rc;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    double *partial = g_divb_static_ptr[dev];
+    Grid g;
+    g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+    g.s[0] = 1; g.s[1] = nx; g.s[2] = nx * ny;          // ntiles <= 65536 bounds N by 2^24
+    g.N = (long long)nx * ny * nz;
+    for (int d = 0; d < 3; ++d) { g.h[d] = 1.0 / g.n[d]; g.rh[d] = (double)g.n[d]; g.lo[d] = 0; g.hi[d] = g.n[d]; }
+    g.ho = ho ? 1 : 0;
+    g.uct = 1;
+    g.rec = 5;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    k_divb_static<<<(unsigned)ntiles, cell_block(), 0, st>>>(g, (int)ntx, (int)nty, bx_face, by_face, bz_face, div_field, partial);
+    if (max_abs_dev) k_divb_static_finish<<<1, 256, 0, st>>>((int)ntiles, partial, max_abs_dev);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        char msg[160];
+        std::snprintf(msg, sizeof(msg), "echo_div_b_static: launch failed: %s", cudaGetErrorString(e));
+        return divb_static_fail(ECHO_ECUDA, msg);
+    }
+    return ECHO_OK;
+}
+
+}  // extern "C"
