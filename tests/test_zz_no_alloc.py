@@ -117,3 +117,28 @@ def test_static_div_b_allocates_nothing_and_honours_the_limit():
     with pytest.raises(eb.EchoError) as ei:
         eb.div_b_static(*too_big, max_abs=m)
     assert ei.value.code == eb.ECHO_EINVAL and "65536" in str(ei.value)
+
+
+@pytest.mark.gpu
+def test_static_div_b_under_stream_capture():
+    """The use case the entry point exists for: captured into a CUDA graph (no allocation, no synchronisation inside
+    the call), replayed twice on changing inputs."""
+    import torch
+    from paper_2401_03008_b200 import binding as eb
+
+    e = _handle_with_faces(eb, torch, (40, 12, 6), 31, 1.0)
+    bf = [e.field(5 + d) for d in range(3)]
+    out = torch.zeros((6, 12, 40), dtype=torch.float64, device="cuda")
+    m = torch.zeros(1, dtype=torch.float64, device="cuda")
+    assert eb.lib().echo_div_b_static_setup() == 0                # symbol lookup before the capture begins
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        eb.div_b_static(*bf, div_field=out, max_abs=m)
+    for scale in (1.0, 0.25):
+        for f in bf:
+            f.mul_(scale)                                         # the graph reads the handle's fields in place
+        graph.replay()
+        torch.cuda.synchronize()
+        ref_max, ref_field = e.div_b(want_field=True)
+        assert float((out - ref_field).abs().max()) <= TOL * ref_max
+        assert abs(float(m[0]) - ref_max) <= TOL * ref_max
