@@ -33,10 +33,11 @@
 // zero-gradient outflow (copy of the nearest interior value).  DESIGN.md section 12.
 //
 // Pins (tests/test_oracle_*.py): see the list in DESIGN.md §"Oracle pins".
-// parity unpinned: inside the MP5 limiter branch, the published design constants 1/2 (v^MD), 4/3 (v^LC) and 4
-// (inside d^M4) against nearby values.  The paper prints nothing that fixes them; what IS pinned about the branch
+// parity unpinned: inside the MP5 limiter branch, the published design constants 4/3 (v^LC) and 4 (inside d^M4)
+// against nearby values.  The paper prints nothing that fixes them; what IS pinned about the branch
 // (tests/test_oracle_units.py, tests/test_oracle_mp5_advection.py): its bounds and symmetries, monotone advection
-// of a pulse at Courant number 1/(1+alpha), transparency on resolved smooth extrema, the bound v_j + alpha dv.
+// of a pulse at Courant number 1/(1+alpha), transparency on resolved smooth extrema, the bound v_j + alpha dv, and
+// the 1/2 of v^MD (with d^M4 = d_{i+1} the bound is the linear extrapolation to the face from the right).
 
 #include <cmath>
 #include <cstddef>

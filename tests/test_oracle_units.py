@@ -108,6 +108,29 @@ def test_mp5_limiter_invariants():
         assert ob.mp5(v + 3.0) == pytest.approx(ob.mp5(v) + 3.0, abs=1e-9)
 
 
+def test_mp5_median_bound_is_the_linear_extrapolation_from_the_right():
+    """The constant 1/2 of v^MD (O3).  v^MD = v^AV - d^M4/2 is Suresh & Huynh's median of v_i, v_{i+1} and the value
+    extrapolated linearly to the face from the right, v^FR = v_{i+1} + (v_{i+1} - v_{i+2})/2: with d^M4 = d_{i+1} the
+    two are the same number, (v_i + v_{i+1})/2 - (v_i - 2 v_{i+1} + v_{i+2})/2 = v^FR.  On the stencils below the
+    unlimited value lies beyond that bound, d^M4_{i+1/2} = d_{i+1} and the other bound (v^UL, v^LC) is wider, so MP5
+    must return v^FR exactly; with 1 or 1/4 in place of 1/2 it returns something else by more than 0.02."""
+    cases = [[-1.8, 1.56, 0.87, 0.79, 0.93], [1.59, -1.65, -1.59, -0.69, 0.63],
+             [-1.94, 1.22, 0.44, 0.45, 0.73], [1.98, -1.43, -0.23, -0.04, -0.21]]
+    for v in cases:
+        v = np.array(v)
+        fr = v[3] + 0.5 * (v[3] - v[4])
+        vor = np.dot([3, -20, 90, 60, -5], v) / 128.0
+        dj, dj1 = v[1] - 2 * v[2] + v[3], v[2] - 2 * v[3] + v[4]
+        # the premises, from the data alone: d_{i+1} is the minmod of (4 d_i - d_{i+1}, 4 d_{i+1} - d_i, d_i, d_{i+1})
+        four = np.array([4 * dj - dj1, 4 * dj1 - dj, dj, dj1])
+        assert (np.sign(four) == np.sign(dj1)).all() and np.abs(four).min() == abs(dj1)
+        assert abs(vor - fr) > 0.05                       # the unlimited value is somewhere else
+        for sgn in (1.0, -1.0):                           # and the odd image
+            assert ob.mp5(sgn * v) == pytest.approx(sgn * fr, abs=2e-15)
+        vav = 0.5 * (v[2] + v[3])
+        assert min(abs(vav - 1.0 * dj1 - fr), abs(vav - 0.25 * dj1 - fr)) > 0.02
+
+
 def test_mp5_clips_overshoot_of_the_linear_scheme():
     # data with a kink where the unlimited quartic overshoots: the limited value must differ from it
     v = np.array([0.0, 0.0, 0.0, 1.0, 2.0])
