@@ -147,3 +147,36 @@ def test_512_x_aligned_sampled_parity():
     assert d1["max_div_b"] * (1.0 / n) <= 1e-12 * 2.0
     for k in ("sum_D", "sum_Sx", "sum_Sy", "sum_Sz", "sum_U", "sum_Bx", "sum_By", "sum_Bz"):
         assert abs(d1[k] - d0[k]) <= 1e-12 * max(abs(d0[k]), 1.0), k
+
+
+def test_640_diag_sampled_parity():
+    """The largest grid of the suite: 640^3 (2.6e8 cells, 92 GB workspace, about 135 GB of device memory at the peak of
+    this test), where every sweep axis is longer than the 512-cell chunk limit (two chunks per column) and the
+    plane-marching kernels run 3-4 z-chunks.  One step of the diagonal wave, sampled sub-boxes recomputed by the
+    oracle (one of them across a z-chunk seam), div B and conservation.  Skipped on a device with less free memory."""
+    import torch
+    from paper_2401_03008_b200 import binding as eb
+    from oracle import binding as ob
+
+    torch.cuda.empty_cache()
+    if torch.cuda.mem_get_info()[0] < 150e9:
+        pytest.skip("needs 150 GB of free device memory")
+    n = 640
+    w = inputs.cpa_wave(n, n, n)
+    e = eb.Echo(n, n, n, G, 0.3)
+    e.set_primitives(*[torch.as_tensor(w[k], device="cuda") for k in SETK])
+    d0 = e.diagnostics()
+    e.step(1)
+    d1 = e.diagnostics()
+    assert d1["rc"] == 0 and d1["steps"] == 1
+    dt = d1["dt_last"]
+    assert dt == pytest.approx(0.3 / n / d1["amax"], rel=1e-14)
+    q = {k: v.cpu().numpy() for k, v in e.get_primitives().items()}
+    seams, til = seam_planes(e)
+    assert til["cx_flux"] < n and til["cy_flux"] < n and til["cz_flux"] < n        # multi-chunk sweeps on all three axes
+    subbox_check(ob, w, q, n, dt, [(0, 0, 0), (n - 1, 300, seams[0] if seams else 100), (til["cx_flux"], n - 1, til["cz_flux"])])
+    assert d1["max_div_b"] * (1.0 / n) <= 1e-12 * 2.0
+    for k in ("sum_D", "sum_Sx", "sum_Sy", "sum_Sz", "sum_U", "sum_Bx", "sum_By", "sum_Bz"):
+        assert abs(d1[k] - d0[k]) <= 1e-12 * max(abs(d0[k]), 1.0), k
+    del e, q, w
+    torch.cuda.empty_cache()
