@@ -4,7 +4,9 @@ entry point has run on grids whose sizes are multiples of nothing (ragged tiles,
 switch the TMA path off, even ones that switch it on, a one-plane grid, a padded block with physical boundaries) the
 bands must be untouched.  A kernel that stores one element past a field, a tile tail that is not masked, a halo
 message one slab too long: each of them lands in a band or in a neighbouring field and shows up here or in the parity
-tests.  Reads cannot be caught this way; the parity tests on the same shapes are the check for those."""
+tests.  The pattern is 0xFF, a NaN when read as a double, and the workspace itself starts out filled with it: a READ
+of a band, of the padding between fields or of a scratch field that no kernel has written yet turns the state into NaN
+and fails the finiteness checks below (the stand-in for initcheck)."""
 import ctypes as C
 
 import numpy as np
@@ -15,7 +17,7 @@ from paper_2401_03008_b200 import inputs
 pytestmark = pytest.mark.gpu
 G = 4.0 / 3.0
 BAND = 1 << 20            # bytes on each side of a guarded buffer (a multiple of 256: the workspace alignment)
-PATTERN = 0xA5
+PATTERN = 0xFF           # as doubles: NaN, so that a READ of a band or of never-written workspace poisons the result
 
 
 class Guarded:
@@ -24,7 +26,7 @@ class Guarded:
     def __init__(self, torch, nbytes):
         self.torch = torch
         self.raw = torch.full((BAND + nbytes + BAND,), PATTERN, dtype=torch.uint8, device="cuda")
-        self.body = self.raw[BAND:BAND + nbytes]
+        self.body = self.raw[BAND:BAND + nbytes]       # starts out as NaN as well (initcheck: see the module docstring)
         assert self.body.data_ptr() % 256 == 0
 
     def intact(self):
@@ -87,8 +89,10 @@ def test_no_write_outside_the_workspace_or_the_outputs(shape, kw):
     e.step(2)                                    # graph replay
     e.use_graph(False)
     e.step(1)                                    # plain launches
-    e.rhs()
-    e.div_b(want_field=True)
+    r = e.rhs()
+    assert all(bool(torch.isfinite(t).all()) for k in ("rhsU", "rhsB", "E") for t in r[k]) and np.isfinite(r["amax"])
+    mdiv, fdiv = e.div_b(want_field=True)
+    assert np.isfinite(mdiv) and bool(torch.isfinite(fdiv).all())
     d = e.diagnostics()
     assert d["rc"] == 0 and d["steps"] == 3 and d["c2p_failures"] == 0
     assert gws.intact()
