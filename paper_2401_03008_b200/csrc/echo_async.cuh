@@ -1,7 +1,7 @@
-// echo_async.cuh — sm_100a asynchronous-copy primitives used by the tile-marching kernels: 1-D bulk copies
-// global -> shared issued by single threads (cp.async.bulk, SASS UBLKCP) that complete on a shared-memory mbarrier
-// by transaction bytes (SASS SYNCS), and the classic per-thread 8-byte cp.async (LDGSTS) kept for grids whose rows
-// are not 16-byte aligned.  Plain wrappers around the PTX; no arithmetic of the method.
+// echo_async.cuh — sm_100a asynchronous-copy primitives used by the tile-marching kernels: TMA box copies
+// global -> shared issued by ONE thread (cp.async.bulk.tensor, SASS UTMALDG) that complete on a shared-memory mbarrier
+// by transaction bytes (SASS SYNCS), and the classic per-thread 8-byte cp.async (LDGSTS), which can arrive on the same
+// mbarrier, for tiles that wrap around a periodic seam.  Plain wrappers around the PTX; no arithmetic of the method.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -28,9 +28,6 @@ __device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 // blocks until the phase of the given parity has completed (try_wait suspends the thread in hardware between polls)
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
     asm volatile(
@@ -43,14 +40,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
         "MBAR_DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
-}
-
-// ---- 1-D bulk copy global -> shared: `bytes` (a multiple of 16) from a 16-byte aligned global address to a 16-byte
-// aligned shared address, issued by ONE thread; completion is signalled on `bar` as `bytes` transaction bytes.
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, unsigned bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
-                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
 }
 
 // ---- TMA: one thread copies a whole 3-D box {bx, by, 1} of a field (tensor map = CUtensorMap in kernel-parameter

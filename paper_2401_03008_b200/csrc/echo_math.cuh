@@ -75,10 +75,10 @@ __device__ __forceinline__ double minmod4(double a, double b, double c, double d
     return diff >= 0 ? m : 0.0;
 }
 
-// O3 — REC: MP5 (Suresh & Huynh 1997) on POINT values.  Left-biased value at i+1/2
-// from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (S2).  The unlimited 5-point value and the S&H test
-// come first; the limiter proper is evaluated (inline, branch) only where the test fires: on smooth
-// data that is the few cells around each extremum.
+// O3 — REC: MP5 (Suresh & Huynh 1997) on POINT values, left-biased value at i+1/2 from v_{i-2..i+2};
+// alpha = 4, eps = 1e-10 (S2).  The unlimited 5-point value vor = (3, -20, 90, 60, -5)/128 . v and the S&H test
+// (vor - v_i)(vor - v^MP) > eps come first (mp5_pair, mp5_pair_fast below, two sides at a time); mp5_limit is the
+// limiter proper, evaluated only where the test fires: on smooth data that is the few cells around each extremum.
 __device__ __forceinline__ double mp5_limit(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
     const double dm1 = fma(-2.0, vm1, vm2) + v0;
     const double d0 = fma(-2.0, v0, vm1) + vp1;
@@ -103,35 +103,6 @@ __device__ __forceinline__ double mp5_limit(double vm2, double vm1, double v0, d
 __device__ __noinline__ double mp5_limit_call(double vm2, double vm1, double v0, double vp1, double vp2, double vor) {
     return mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
 }
-// the same behind the exact S&H test (for callers that flagged the stencil with a cheaper superset of it)
-__device__ __noinline__ double mp5_limit_call_checked(double vm2, double vm1, double v0, double vp1, double vp2,
-                                                      double vor) {
-    const double t = vor - v0;
-    const double a = vp1 - v0, b = 4.0 * (v0 - vm1);
-    const double m = (fabs(a) < fabs(b)) ? a : b;
-    const double mm = ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
-    if (!(t * (t - mm) > 1e-10)) return vor;
-    return mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
-}
-// INL: limiter inlined behind a branch (flux sweeps) or called out of line (UCT kernel, whose 24
-// reconstructions would otherwise overflow the instruction cache).
-template <bool INL = true>
-__device__ __forceinline__ double mp5(double vm2, double vm1, double v0, double vp1, double vp2) {
-    const double vor = (3.0 / 128.0) * vm2 + ((-20.0 / 128.0) * vm1 + ((90.0 / 128.0) * v0 +
-                       ((60.0 / 128.0) * vp1 + (-5.0 / 128.0) * vp2)));
-    const double vmp = v0 + minmod2(vp1 - v0, 4.0 * (v0 - vm1));
-    double r = vor;
-    if ((vor - v0) * (vor - vmp) > 1e-10) {
-        if (INL) {
-            asm volatile("" ::: "memory");   // keeps this a real branch: the limiter must not be if-converted
-            r = mp5_limit(vm2, vm1, v0, vp1, vp2, vor);
-        } else {
-            r = mp5_limit_call(vm2, vm1, v0, vp1, vp2, vor);
-        }
-    }
-    return r;
-}
-
 // Both one-sided values at the face between s2 and s3 from the six cells s0..s5 around it:
 // L = MP5(s0..s4) centred on s2, R = MP5(s5..s1) centred on s3 (mirrored).  The S&H test is evaluated
 // as t (t - mm) > eps with t = vOR - v_i and mm = minmod(v_{i+1} - v_i, 4 (v_i - v_{i-1})): the two sides
@@ -140,9 +111,9 @@ __device__ __forceinline__ double mp5(double vm2, double vm1, double v0, double 
 __device__ __forceinline__ double times4(double d) {
     return __hiloint2double(__double2hiint(d) + 0x00200000, __double2loint(d));
 }
+// INL: limiter inlined behind a branch (flux sweeps) or called out of line.
 #ifndef ECHO_SH_SUPERSET
 #define ECHO_SH_SUPERSET 1       // sweeps: x 0.785 -> 0.776, y 0.757 -> 0.741, z 0.808 -> 0.804 ms at 256^3
-#define ECHO_SH_SUPERSET_UCT 0   // UCT kernel: 1.16 -> 1.19-1.22 ms with it (inline or behind the checked call)
 #endif
 template <bool INL = true>
 __device__ __forceinline__ void mp5_pair(double s0, double s1, double s2, double s3, double s4, double s5, double &L,
@@ -219,25 +190,15 @@ __device__ __forceinline__ unsigned mp5_pair_fast(double s0, double s1, double s
     R = (3.0 / 128.0) * s5 + ((-20.0 / 128.0) * s4 + ((90.0 / 128.0) * s3 + ((60.0 / 128.0) * s2 + (-5.0 / 128.0) * s1)));
     const double d23 = s3 - s2;
     const double tL = L - s2, tR = R - s3;
-#if ECHO_SH_SUPERSET_UCT
-    // superset of the S&H test (see mp5_pair); mp5_pair_fix repeats the exact test
-    return ((tL * (tL - d23) > 1e-10 || tL * fma(-4.0, s2 - s1, tL) > 1e-10) ? 1u : 0u) |
-           ((tR * (tR + d23) > 1e-10 || tR * fma(-4.0, s3 - s4, tR) > 1e-10) ? 2u : 0u);
-#else
+    // the exact S&H test: its select-free superset (mp5_pair) makes the UCT kernel slower (1.16 -> 1.19-1.22 ms)
     const double mmL = minmod2(d23, times4(s2 - s1));
     const double mmR = minmod2(-d23, times4(s3 - s4));
     return (tL * (tL - mmL) > 1e-10 ? 1u : 0u) | (tR * (tR - mmR) > 1e-10 ? 2u : 0u);
-#endif
 }
 __device__ __forceinline__ void mp5_pair_fix(unsigned bits, double s0, double s1, double s2, double s3, double s4,
                                              double s5, double &L, double &R) {
-#if ECHO_SH_SUPERSET_UCT
-    if (bits & 1u) L = mp5_limit_call_checked(s0, s1, s2, s3, s4, L);
-    if (bits & 2u) R = mp5_limit_call_checked(s5, s4, s3, s2, s1, R);
-#else
     if (bits & 1u) L = mp5_limit_call(s0, s1, s2, s3, s4, L);
     if (bits & 2u) R = mp5_limit_call(s5, s4, s3, s2, s1, R);
-#endif
 }
 
 // ---------------------------------------------------------------- point physics
